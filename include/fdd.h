@@ -1,0 +1,162 @@
+/* fdd.h -- C ABI of the B200-native Fourier-domain dedispersion (FDD) hot path.
+ *
+ * Method: Bassa, Romein, Veenboer, van der Vlugt & Wijnholds, "Fourier-domain dedispersion",
+ * arXiv:2110.03482.  Citations "PAPER.md:<line>" refer to the paper text the build was given.
+ *
+ * One fdd_execute() call runs, on one GPU and one CUDA stream, with no host synchronisation:
+ *
+ *   a2  unpack + transpose (+ zero pad)   u8 [nsamps][nchans] -> f32 [nchans][nfft]
+ *                                          (Algorithm 1 lines 10-11)
+ *   a3  batched real-to-complex FFT        X[c][k] = sum_n x[c][n] e^{-2 pi i k n / nfft}
+ *                                          (Eq. 3; cuFFT)
+ *   a4  phase-rotate-and-sum               Y[j][k] = sum_c X[c][k] e^{+2 pi i k d[j][c] / nfft}
+ *                                          (Eq. 4 + Eq. 7; the hot kernel)
+ *   a5  TIME:    batched complex-to-real FFT and 1/nfft scaling (Eq. 6)
+ *       FOURIER: nothing -- Y is the output (periodicity searches)
+ *
+ * with the delay table (a1, Eq. 1, against the highest channel)
+ *
+ *   d[j][c] = k_dm * dm_j * (nu_c^-2 - f_hi^-2) / tsamp   [samples],
+ *   nu_c    = f_lo + c (f_hi - f_lo) / (nchans - 1)       [MHz]   (nu_0 = f_hi if nchans == 1)
+ *
+ * built once per plan on the host in long double.  nfft is the next power of two >= nsamps
+ * (PAPER.md:155).  Sign convention: y_j[n] = sum_c x_c[(n + d[j][c]) mod nfft] (band-limited
+ * for fractional d), i.e. dispersed pulses are re-aligned at the arrival time of the highest
+ * channel; with the forward kernel e^{-2 pi i k n / nfft} of Eq. 3 that is the phasor
+ * e^{+2 pi i k d / nfft}.  (Eq. 4's literal minus sign belongs to the opposite transform
+ * sign; the two give conjugate spectra and identical time series.  DESIGN.md, reading S1.)
+ *
+ * Conventions
+ *   - All pointers named "host" are host memory, all named "dev"/in_u8/out (fdd_execute) are
+ *     DEVICE memory of the current CUDA device.  The caller owns in_u8 and out; the plan owns
+ *     every table, scratch buffer, cuFFT plan and workspace.  in_u8 is never modified.
+ *   - A plan belongs to the device that was current at creation and is not re-entrant: at most
+ *     one execute in flight per plan.  Different plans may run concurrently.
+ *   - Every function returns FDD_OK (0) or a negative fdd_status; nothing throws, nothing
+ *     prints, no global state.  A failed create leaves *plan_out = NULL and frees everything.
+ *   - There is no CPU fallback: without a CUDA device fdd_plan_create returns FDD_ERR_CUDA.
+ */
+#ifndef FDD_H_
+#define FDD_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdd_plan fdd_plan;   /* opaque */
+
+enum fdd_mode {
+    FDD_MODE_TIME = 0,      /* out = float32 [ndm][nsamps], includes the 1/nfft of Eq. 6          */
+    FDD_MODE_FOURIER = 1    /* out = float2  [ndm][nfft/2+1] (re, im), unnormalised Y of Eq. 7    */
+};
+
+enum fdd_status {
+    FDD_OK = 0,
+    FDD_ERR_INVALID_ARG = -1,
+    FDD_ERR_ALLOC = -2,
+    FDD_ERR_CUDA = -3,
+    FDD_ERR_CUFFT = -4,
+    FDD_ERR_UNSUPPORTED = -5
+};
+
+/* Kernel choice for step a4 (fdd_plan_set_kernel). */
+enum fdd_kernel {
+    FDD_KERNEL_AUTO = 0,       /* symmetric kernel where the DM grid allows it, else generic     */
+    FDD_KERNEL_GENERIC = 1,    /* any delay table: one exactly range-reduced phasor per element  */
+    FDD_KERNEL_SYMMETRIC = 2   /* DM tiles in arithmetic progression: paired +-m rows */
+};
+
+/* Stage indices for fdd_plan_get_stage_ms. */
+enum fdd_stage {
+    FDD_STAGE_UNPACK = 0, FDD_STAGE_R2C = 1, FDD_STAGE_ROTATE_SUM = 2, FDD_STAGE_C2R = 3,
+    FDD_NUM_STAGES = 4
+};
+
+/* a1. Create a plan for nchans channels whose centres run evenly from f_lo_mhz (channel 0) to
+ * f_hi_mhz (channel nchans-1), nsamps time samples of tsamp_s seconds, and the trial DMs
+ * dm_list_host[0..ndm) in pc cm^-3 (HOST pointer, copied; any finite values, any order).
+ * Requires nchans >= 1, nsamps >= 2, tsamp_s > 0, 0 < f_lo_mhz <= f_hi_mhz, ndm >= 1.
+ * Dispersion constant k_dm = 4.148808e3 MHz^2 pc^-1 cm^3 s (fdd_plan_set_kdm to change).
+ * Allocates all device scratch (see fdd_plan_get_info for the size). */
+int fdd_plan_create(fdd_plan **plan_out, int nchans, long long nsamps, double tsamp_s,
+                    double f_lo_mhz, double f_hi_mhz, const double *dm_list_host, int ndm);
+
+/* Same, from an explicit delay table delay_samples_host[ndm][nchans] (HOST, row-major, in
+ * samples, any finite values) instead of frequencies and DMs.  Integer delays make the result
+ * an exact circular shift-and-sum, which is how the tests pin the kernels without any FFT in
+ * the reference. */
+int fdd_plan_create_from_delays(fdd_plan **plan_out, int nchans, long long nsamps,
+                                const double *delay_samples_host, int ndm);
+
+/* Rebuild the delay and phase tables with another dispersion constant (Eq. 1's k_DM; the paper
+ * quotes (2.41e-4)^-1 = 4149.378).  Only for plans made by fdd_plan_create. Synchronises the
+ * device (it re-uploads tables the previous execute may still be reading). */
+int fdd_plan_set_kdm(fdd_plan *plan, double k_dm);
+
+/* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
+ * for a delay table that is not in arithmetic progression within every DM tile. */
+int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
+
+/* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy
+ * default stream).
+ *   in_u8  DEVICE, uint8 [nsamps][nchans], channel fastest, channel 0 = f_lo
+ *   out    DEVICE, TIME:    float  [ndm][nsamps]; all nsamps samples of the circular result are
+ *                           written, the first valid_len are free of wrap-around
+ *                  FOURIER: float2 [ndm][nfft/2+1]; equals the forward DFT (kernel
+ *                           e^{-2 pi i k n/nfft}) of the full-length circular TIME row times nfft/nfft,
+ *                           i.e. unnormalised; bins 0 and nfft/2 keep their imaginary parts.
+ * Errors: FDD_ERR_INVALID_ARG (NULL pointers, bad mode), FDD_ERR_CUDA / FDD_ERR_CUFFT with the
+ * output undefined. */
+int fdd_execute(fdd_plan *plan, const unsigned char *in_u8, void *out, int mode,
+                void *cuda_stream);
+
+/* End-to-end convenience for HOST buffers: copies in_host (uint8 [nsamps][nchans]) to the
+ * device, runs fdd_execute, copies the result to out_host (layout as fdd_execute's out), and
+ * returns after the result has landed (synchronises cuda_stream).  Pinned host memory makes
+ * the copies asynchronous and overlapped with compute (TIME mode copies finished DM chunks
+ * back while later chunks are still being transformed, as Algorithm 1 lines 19-22 do);
+ * pageable memory works but is slower.  Staging buffers are plan-owned and
+ * allocated on first use. */
+int fdd_execute_host(fdd_plan *plan, const unsigned char *in_host, void *out_host, int mode,
+                     void *cuda_stream);
+
+/* Free everything the plan owns.  NULL is a no-op returning FDD_OK. */
+int fdd_plan_destroy(fdd_plan *plan);
+
+/* Any output pointer may be NULL.  valid_len = nsamps - ceil(max |d|);
+ * scratch_bytes = device memory the plan holds; kernel = the a4 kernel in use (enum fdd_kernel,
+ * never AUTO). */
+int fdd_plan_get_info(const fdd_plan *plan, long long *nfft, long long *nbins,
+                      long long *valid_len, double *max_delay_samples, size_t *scratch_bytes,
+                      int *kernel);
+
+/* Copy the plan's delay table to delay_samples_host[ndm][nchans] (HOST). */
+int fdd_plan_get_delays(const fdd_plan *plan, double *delay_samples_host);
+
+/* Stage timing.  fdd_plan_set_profiling(plan, 1) makes fdd_execute record CUDA events between
+ * the stages on its stream; fdd_plan_get_stage_ms then waits for the last execute and writes
+ * the device time of each stage in milliseconds to ms_host[FDD_NUM_STAGES] (0 for a skipped
+ * stage) and, if launches_host != NULL, how many kernels/library calls each stage launched. */
+int fdd_plan_set_profiling(fdd_plan *plan, int enable);
+int fdd_plan_get_stage_ms(fdd_plan *plan, float *ms_host, int *launches_host);
+
+/* Debug/test access: DEVICE pointer to the channel spectra X (float2 [nchans][pitch]) left by
+ * the last execute, and the row pitch in float2 elements. */
+int fdd_plan_get_spectrum(const fdd_plan *plan, void **x_dev, long long *pitch_elems);
+
+/* Run only a4 on the spectra left by the last execute (for timing sweeps of the hot kernel). */
+int fdd_rotate_sum_only(fdd_plan *plan, void *out, int mode, void *cuda_stream);
+
+/* Measure this device's FP32 FMA rate with a register-resident FFMA loop on every SM (the
+ * denominator of the a4 roofline).  packed != 0 uses fma.rn.f32x2.  Writes
+ * TFLOP/s (2 flop per FMA lane) and the kernel time.  Synchronous. */
+int fdd_measure_fp32_peak(int packed, int iters, double *tflops_host, float *ms_host);
+
+const char *fdd_error_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDD_H_ */

@@ -1,0 +1,717 @@
+// C ABI of the FDD hot path (include/fdd.h): plan tables, scratch, cuFFT plans, stage launches.
+// Everything numerical on the device happens in the kernels of fdd_kernels_*.cuh and in cuFFT
+// (allowed for the FFT stages); the host only builds the phase tables.
+#include "../../include/fdd.h"
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "fdd_kernels_generic.cuh"
+#include "fdd_kernels_pre.cuh"
+#include "fdd_kernels_sym.cuh"
+
+namespace {
+
+constexpr double kDefaultKdm = 4.148808e3;            // MHz^2 pc^-1 cm^3 s (reading S5)
+constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
+constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
+constexpr int kC2RBatch = 256;                        // rows per cuFFT C2R call (bounds workspace)
+
+inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
+
+struct StageEvent {
+    int stage;
+    cudaEvent_t beg, end;
+};
+
+}  // namespace
+
+struct fdd_plan {
+    // problem
+    int nchans = 0, ndm = 0;
+    long long nsamps = 0, nfft = 0, nbins = 0;
+    double tsamp = 0, f_lo = 0, f_hi = 0, kdm = kDefaultKdm;
+    bool from_delays = false;
+    std::vector<double> dm_list;
+    std::vector<double> delays;          // [ndm][nchans], samples
+    double max_delay = 0;
+    long long valid_len = 0;
+    int device = 0;
+    // device buffers
+    float2* X = nullptr;                 // [nchans][xpitch]; also the real rows of the in-place R2C
+    long long xpitch = 0;
+    float2* Y = nullptr;                 // TIME mode: [y_rows][ypitch] (lazily allocated)
+    long long ypitch = 0;
+    int y_rows = 0;
+    unsigned long long* phase64 = nullptr;   // generic kernel: [nchans][ndm_pad]
+    int ndm_pad = 0;
+    fdd::SymTables sym;                  // symmetric kernel tables (device) + tiling
+    bool sym_ok = false;
+    int kernel = FDD_KERNEL_GENERIC;     // resolved choice
+    int kernel_request = FDD_KERNEL_AUTO;
+    // FFT
+    cufftHandle r2c = 0, c2r = 0, c2r_tail = 0;
+    bool have_r2c = false, have_c2r = false, have_c2r_tail = false;
+    int c2r_batch = 0, c2r_tail_batch = 0;
+    void* fft_ws = nullptr;
+    size_t fft_ws_bytes = 0;
+    // host staging (fdd_execute_host)
+    unsigned char* stage_in = nullptr;
+    void* stage_out = nullptr;
+    size_t stage_out_bytes = 0;
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> chunk_events;
+    // profiling
+    bool profiling = false;
+    std::vector<StageEvent> events;
+    size_t events_used = 0;
+    int launches[FDD_NUM_STAGES] = {0, 0, 0, 0};
+    size_t scratch_bytes = 0;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard()
+    {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+
+template <class T>
+int dev_alloc(fdd_plan* p, T** ptr, size_t count)
+{
+    void* v = nullptr;
+    const size_t bytes = count * sizeof(T);
+    if (cudaMalloc(&v, bytes ? bytes : 1) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_ALLOC;
+    }
+    *ptr = static_cast<T*>(v);
+    p->scratch_bytes += bytes;
+    return FDD_OK;
+}
+
+// a1: delay table from frequencies and DMs (Eq. 1), in long double.
+void build_delays(fdd_plan* p)
+{
+    p->delays.assign((size_t)p->ndm * p->nchans, 0.0);
+    const long double fhi = p->f_hi;
+    for (int c = 0; c < p->nchans; ++c) {
+        const long double nu =
+            p->nchans == 1 ? fhi
+                           : (long double)p->f_lo +
+                                 (long double)c * ((long double)p->f_hi - (long double)p->f_lo) /
+                                     (long double)(p->nchans - 1);
+        const long double per_dm =
+            (long double)p->kdm * (1.0L / (nu * nu) - 1.0L / (fhi * fhi)) / (long double)p->tsamp;
+        for (int j = 0; j < p->ndm; ++j)
+            p->delays[(size_t)j * p->nchans + c] = (double)((long double)p->dm_list[j] * per_dm);
+    }
+}
+
+void finish_delay_stats(fdd_plan* p)
+{
+    double m = 0;
+    for (double d : p->delays) m = fmax(m, fabs(d));
+    p->max_delay = m;
+    // S10: mathematically integer delays may evaluate a hair above the integer
+    p->valid_len = p->nsamps - (long long)ceil(m * (1.0 - 1e-12));
+}
+
+// frac(d / nfft) as a 64-bit binary fraction of a cycle.
+inline unsigned long long cycles_to_fixed64(long double cyc)
+{
+    long double f = cyc - floorl(cyc);                   // [0, 1)
+    long double s = f * 18446744073709551616.0L;         // * 2^64
+    if (s >= 18446744073709551615.0L) return 0ULL;       // rounds up to a whole cycle
+    return (unsigned long long)(s + 0.5L);
+}
+
+int upload_generic_table(fdd_plan* p)
+{
+    std::vector<unsigned long long> tab((size_t)p->nchans * p->ndm_pad, 0ULL);
+    for (int j = 0; j < p->ndm; ++j)
+        for (int c = 0; c < p->nchans; ++c)
+            tab[(size_t)c * p->ndm_pad + j] = cycles_to_fixed64(
+                (long double)p->delays[(size_t)j * p->nchans + c] / (long double)p->nfft);
+    if (cudaMemcpy(p->phase64, tab.data(), tab.size() * sizeof(unsigned long long),
+                   cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_CUDA;
+    }
+    return FDD_OK;
+}
+
+int build_tables(fdd_plan* p)
+{
+    finish_delay_stats(p);
+    int rc = upload_generic_table(p);
+    if (rc != FDD_OK) return rc;
+    rc = fdd::sym_build_tables(&p->sym, p->delays.data(), p->ndm, p->nchans, p->nfft, &p->sym_ok,
+                               &p->scratch_bytes);
+    if (rc != FDD_OK) return rc;
+    p->kernel = (p->kernel_request == FDD_KERNEL_GENERIC || !p->sym_ok) ? FDD_KERNEL_GENERIC
+                                                                        : FDD_KERNEL_SYMMETRIC;
+    return FDD_OK;
+}
+
+int make_fft_plans(fdd_plan* p)
+{
+    // R2C, in place: real rows of pitch 2*xpitch floats, complex rows of pitch xpitch.
+    size_t ws_r2c = 0;
+    if (cufftCreate(&p->r2c) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    p->have_r2c = true;
+    if (cufftSetAutoAllocation(p->r2c, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    long long n[1] = {p->nfft};
+    long long inembed[1] = {2 * p->xpitch}, onembed[1] = {p->xpitch};
+    if (cufftMakePlanMany64(p->r2c, 1, n, inembed, 1, 2 * p->xpitch, onembed, 1, p->xpitch,
+                            CUFFT_R2C, p->nchans, &ws_r2c) != CUFFT_SUCCESS)
+        return FDD_ERR_CUFFT;
+    p->fft_ws_bytes = ws_r2c;
+    return FDD_OK;
+}
+
+int make_c2r_plan(fdd_plan* p, cufftHandle* h, int batch, size_t* ws)
+{
+    if (cufftCreate(h) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    if (cufftSetAutoAllocation(*h, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    long long n[1] = {p->nfft};
+    const bool direct = (p->nsamps == p->nfft);     // straight into the caller's rows
+    long long inembed[1] = {p->ypitch};
+    long long onembed[1] = {direct ? p->nfft : 2 * p->ypitch};
+    const long long odist = direct ? p->nfft : 2 * p->ypitch;
+    if (cufftMakePlanMany64(*h, 1, n, inembed, 1, p->ypitch, onembed, 1, odist, CUFFT_C2R, batch,
+                            ws) != CUFFT_SUCCESS)
+        return FDD_ERR_CUFFT;
+    return FDD_OK;
+}
+
+// TIME-mode resources are allocated on the first TIME execute (a FOURIER-only plan such as
+// config 5 never needs the 16 GiB of Y).
+int ensure_time_resources(fdd_plan* p)
+{
+    if (p->Y) return FDD_OK;
+    p->ypitch = round_up(p->nbins, kPitchAlign);
+    const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
+    long long rows = (long long)(kYBudgetBytes / row_bytes);
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+        long long fit = (long long)(free_b / 2 / row_bytes);
+        if (fit < rows) rows = fit;
+    }
+    if (rows >= p->ndm) rows = p->ndm;
+    else rows = rows / kC2RBatch * kC2RBatch;
+    if (rows < 1) return FDD_ERR_ALLOC;
+    p->y_rows = (int)rows;
+    p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
+    size_t ws_a = 0, ws_b = 0;
+    int rc = make_c2r_plan(p, &p->c2r, p->c2r_batch, &ws_a);
+    p->have_c2r = true;
+    if (rc != FDD_OK) return rc;
+    // tails: of a full Y chunk and of the last (short) chunk; at most one distinct tail size is
+    // planned, any other remainder is issued row by row through it.
+    const int last_rows = p->ndm % p->y_rows ? p->ndm % p->y_rows : p->y_rows;
+    int tail = last_rows % p->c2r_batch;
+    if (tail == 0) tail = p->y_rows % p->c2r_batch;
+    if (tail) {
+        rc = make_c2r_plan(p, &p->c2r_tail, tail, &ws_b);
+        p->have_c2r_tail = true;
+        if (rc != FDD_OK) return rc;
+        p->c2r_tail_batch = tail;
+    }
+    size_t need = ws_a > ws_b ? ws_a : ws_b;
+    if (need > p->fft_ws_bytes) {
+        if (p->fft_ws) { cudaFree(p->fft_ws); p->scratch_bytes -= p->fft_ws_bytes; p->fft_ws = nullptr; }
+        p->fft_ws_bytes = need;
+        rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->fft_ws), need);
+        if (rc != FDD_OK) return rc;
+        if (cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    }
+    if (cufftSetWorkArea(p->c2r, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    if (p->have_c2r_tail && cufftSetWorkArea(p->c2r_tail, p->fft_ws) != CUFFT_SUCCESS)
+        return FDD_ERR_CUFFT;
+    return dev_alloc(p, &p->Y, (size_t)p->y_rows * p->ypitch);
+}
+
+void destroy_plan(fdd_plan* p)
+{
+    if (!p) return;
+    DeviceGuard g(p->device);
+    cudaDeviceSynchronize();
+    if (p->have_r2c) cufftDestroy(p->r2c);
+    if (p->have_c2r) cufftDestroy(p->c2r);
+    if (p->have_c2r_tail) cufftDestroy(p->c2r_tail);
+    cudaFree(p->X);
+    cudaFree(p->Y);
+    cudaFree(p->phase64);
+    cudaFree(p->fft_ws);
+    cudaFree(p->stage_in);
+    cudaFree(p->stage_out);
+    fdd::sym_free_tables(&p->sym);
+    for (auto& e : p->events) { cudaEventDestroy(e.beg); cudaEventDestroy(e.end); }
+    for (auto& e : p->chunk_events) cudaEventDestroy(e);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    cudaGetLastError();
+    delete p;
+}
+
+int create_common(fdd_plan* p)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return FDD_ERR_CUDA; }
+    if (cudaGetDevice(&p->device) != cudaSuccess) return FDD_ERR_CUDA;
+    p->nfft = 2;
+    while (p->nfft < p->nsamps) p->nfft <<= 1;
+    p->nbins = p->nfft / 2 + 1;
+    p->xpitch = round_up(p->nbins, kPitchAlign);
+    p->ndm_pad = (int)round_up(p->ndm, fdd::kGenDT);
+    int rc = dev_alloc(p, &p->X, (size_t)p->nchans * p->xpitch);
+    if (rc != FDD_OK) return rc;
+    rc = dev_alloc(p, &p->phase64, (size_t)p->nchans * p->ndm_pad);
+    if (rc != FDD_OK) return rc;
+    rc = build_tables(p);
+    if (rc != FDD_OK) return rc;
+    rc = make_fft_plans(p);
+    if (rc != FDD_OK) return rc;
+    if (p->fft_ws_bytes) {
+        size_t need = p->fft_ws_bytes;
+        p->fft_ws_bytes = 0;
+        rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->fft_ws), need);
+        if (rc != FDD_OK) return rc;
+        p->fft_ws_bytes = need;
+    }
+    if (cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    return FDD_OK;
+}
+
+// ---- profiling helpers -----------------------------------------------------------------
+struct StageTimer {
+    fdd_plan* p;
+    cudaStream_t s;
+    StageEvent* cur = nullptr;
+    StageTimer(fdd_plan* plan, cudaStream_t stream) : p(plan), s(stream) {}
+    void begin(int stage, int launches)
+    {
+        p->launches[stage] += launches;
+        if (!p->profiling) return;
+        if (p->events_used == p->events.size()) {
+            StageEvent e;
+            e.stage = stage;
+            if (cudaEventCreate(&e.beg) != cudaSuccess || cudaEventCreate(&e.end) != cudaSuccess) {
+                cudaGetLastError();
+                return;
+            }
+            p->events.push_back(e);
+        }
+        cur = &p->events[p->events_used++];
+        cur->stage = stage;
+        cudaEventRecord(cur->beg, s);
+    }
+    void end()
+    {
+        if (cur) cudaEventRecord(cur->end, s);
+        cur = nullptr;
+    }
+};
+
+int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
+{
+    dim3 grid((unsigned)((p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile),
+              (unsigned)((p->nchans + fdd::kUnpackTile - 1) / fdd::kUnpackTile));
+    float* xf = reinterpret_cast<float*>(p->X);
+    const bool vec = (p->nchans % 4 == 0) && ((uintptr_t)in_u8 % 4 == 0);
+    if (vec)
+        fdd::k_unpack_transpose<4><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
+                                                        2 * p->xpitch);
+    else
+        fdd::k_unpack_transpose<1><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
+                                                        2 * p->xpitch);
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
+// a4 on DM rows [j_begin, j_begin + rows) into dst (row pitch opitch float2).
+int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
+                      cudaStream_t s)
+{
+    const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
+    const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
+    if (p->kernel == FDD_KERNEL_SYMMETRIC)
+        return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
+                               dst, opitch, scale, real_edges, s);
+    const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
+    const long long n_kt = (p->nbins + fdd::kGenThreads - 1) / fdd::kGenThreads;
+    if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
+    fdd::k_rotate_sum_generic<<<(unsigned)(n_jt * n_kt), fdd::kGenThreads, 0, s>>>(
+        p->X, p->xpitch, p->phase64, p->ndm_pad, p->nchans, p->nbins, j_begin + rows, j_begin, n_jt,
+        dst, opitch, scale, real_edges);
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
+int launch_c2r_rows(fdd_plan* p, int rows, float2* ysrc, float* dst, cudaStream_t s, int* launches)
+{
+    // ysrc: [rows][ypitch]; dst: caller rows (pitch nsamps).
+    const bool direct = (p->nsamps == p->nfft);
+    int done = 0;
+    while (done < rows) {
+        int left = rows - done;
+        cufftHandle h;
+        int b;
+        if (left >= p->c2r_batch) { h = p->c2r; b = p->c2r_batch; }
+        else if (p->have_c2r_tail && left >= p->c2r_tail_batch) { h = p->c2r_tail; b = p->c2r_tail_batch; }
+        else return FDD_ERR_UNSUPPORTED;     // cannot happen: tails are planned in ensure_time_resources
+        if (cufftSetStream(h, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+        float2* src = ysrc + (long long)done * p->ypitch;
+        if (direct) {
+            if (cufftExecC2R(h, src, dst + (long long)done * p->nsamps) != CUFFT_SUCCESS)
+                return FDD_ERR_CUFFT;
+            ++*launches;
+        } else {
+            if (cufftExecC2R(h, src, reinterpret_cast<float*>(src)) != CUFFT_SUCCESS)
+                return FDD_ERR_CUFFT;
+            if (cudaMemcpy2DAsync(dst + (long long)done * p->nsamps, (size_t)p->nsamps * sizeof(float),
+                                  src, (size_t)p->ypitch * sizeof(float2),
+                                  (size_t)p->nsamps * sizeof(float), b, cudaMemcpyDeviceToDevice,
+                                  s) != cudaSuccess)
+                return FDD_ERR_CUDA;
+            *launches += 2;
+        }
+        done += b;
+    }
+    return FDD_OK;
+}
+
+int check_plan(const fdd_plan* p) { return p ? FDD_OK : FDD_ERR_INVALID_ARG; }
+
+// Stages a2+a3.
+int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer& tm)
+{
+    tm.begin(FDD_STAGE_UNPACK, 1);
+    int rc = launch_unpack(p, in_u8, s);
+    tm.end();
+    if (rc != FDD_OK) return rc;
+    tm.begin(FDD_STAGE_R2C, 1);
+    if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    float* xf = reinterpret_cast<float*>(p->X);
+    if (cufftExecR2C(p->r2c, xf, p->X) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    tm.end();
+    return FDD_OK;
+}
+
+// Stages a4+a5 from the spectra in p->X.  chunk_done (optional) is called after each DM chunk
+// has been queued, with (j_begin, rows), so fdd_execute_host can overlap the copy back.
+template <class F>
+int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F chunk_done)
+{
+    if (mode == FDD_MODE_FOURIER) {
+        tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+        int rc = launch_rotate_sum(p, 0, p->ndm, static_cast<float2*>(out), p->nbins, mode, s);
+        tm.end();
+        if (rc == FDD_OK) chunk_done(0, p->ndm);
+        return rc;
+    }
+    int rc = ensure_time_resources(p);
+    if (rc != FDD_OK) return rc;
+    for (int j0 = 0; j0 < p->ndm; j0 += p->y_rows) {
+        const int rows = (p->ndm - j0 < p->y_rows) ? p->ndm - j0 : p->y_rows;
+        tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+        rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s);
+        tm.end();
+        if (rc != FDD_OK) return rc;
+        int nl = 0;
+        tm.begin(FDD_STAGE_C2R, 0);
+        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + (long long)j0 * p->nsamps, s,
+                             &nl);
+        tm.end();
+        p->launches[FDD_STAGE_C2R] += nl;
+        if (rc != FDD_OK) return rc;
+        chunk_done(j0, rows);
+    }
+    return FDD_OK;
+}
+
+void reset_profile(fdd_plan* p)
+{
+    p->events_used = 0;
+    for (int i = 0; i < FDD_NUM_STAGES; ++i) p->launches[i] = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fdd_plan_create(fdd_plan** plan_out, int nchans, long long nsamps, double tsamp_s,
+                    double f_lo_mhz, double f_hi_mhz, const double* dm_list_host, int ndm)
+{
+    if (!plan_out) return FDD_ERR_INVALID_ARG;
+    *plan_out = nullptr;
+    if (nchans < 1 || nsamps < 2 || !(tsamp_s > 0) || !(f_lo_mhz > 0) || !(f_hi_mhz >= f_lo_mhz) ||
+        !isfinite(tsamp_s) || !isfinite(f_hi_mhz) || ndm < 1 || !dm_list_host)
+        return FDD_ERR_INVALID_ARG;
+    for (int j = 0; j < ndm; ++j)
+        if (!isfinite(dm_list_host[j])) return FDD_ERR_INVALID_ARG;
+    fdd_plan* p = new (std::nothrow) fdd_plan();
+    if (!p) return FDD_ERR_ALLOC;
+    p->nchans = nchans; p->nsamps = nsamps; p->tsamp = tsamp_s;
+    p->f_lo = f_lo_mhz; p->f_hi = f_hi_mhz; p->ndm = ndm;
+    p->dm_list.assign(dm_list_host, dm_list_host + ndm);
+    build_delays(p);
+    int rc = create_common(p);
+    if (rc != FDD_OK) { destroy_plan(p); return rc; }
+    *plan_out = p;
+    return FDD_OK;
+}
+
+int fdd_plan_create_from_delays(fdd_plan** plan_out, int nchans, long long nsamps,
+                                const double* delay_samples_host, int ndm)
+{
+    if (!plan_out) return FDD_ERR_INVALID_ARG;
+    *plan_out = nullptr;
+    if (nchans < 1 || nsamps < 2 || ndm < 1 || !delay_samples_host) return FDD_ERR_INVALID_ARG;
+    for (size_t i = 0; i < (size_t)ndm * nchans; ++i)
+        if (!isfinite(delay_samples_host[i])) return FDD_ERR_INVALID_ARG;
+    fdd_plan* p = new (std::nothrow) fdd_plan();
+    if (!p) return FDD_ERR_ALLOC;
+    p->nchans = nchans; p->nsamps = nsamps; p->ndm = ndm; p->from_delays = true;
+    p->delays.assign(delay_samples_host, delay_samples_host + (size_t)ndm * nchans);
+    int rc = create_common(p);
+    if (rc != FDD_OK) { destroy_plan(p); return rc; }
+    *plan_out = p;
+    return FDD_OK;
+}
+
+int fdd_plan_set_kdm(fdd_plan* p, double k_dm)
+{
+    if (check_plan(p) != FDD_OK || !(k_dm > 0) || !isfinite(k_dm)) return FDD_ERR_INVALID_ARG;
+    if (p->from_delays) return FDD_ERR_UNSUPPORTED;
+    DeviceGuard g(p->device);
+    if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
+    p->kdm = k_dm;
+    build_delays(p);
+    return build_tables(p);
+}
+
+int fdd_plan_set_kernel(fdd_plan* p, int kernel)
+{
+    if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
+    if (kernel != FDD_KERNEL_AUTO && kernel != FDD_KERNEL_GENERIC && kernel != FDD_KERNEL_SYMMETRIC)
+        return FDD_ERR_INVALID_ARG;
+    if (kernel == FDD_KERNEL_SYMMETRIC && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
+    p->kernel_request = kernel;
+    p->kernel = (kernel == FDD_KERNEL_GENERIC || !p->sym_ok) ? FDD_KERNEL_GENERIC
+                                                             : FDD_KERNEL_SYMMETRIC;
+    return FDD_OK;
+}
+
+int fdd_execute(fdd_plan* p, const unsigned char* in_u8, void* out, int mode, void* cuda_stream)
+{
+    if (check_plan(p) != FDD_OK || !in_u8 || !out ||
+        (mode != FDD_MODE_TIME && mode != FDD_MODE_FOURIER))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    reset_profile(p);
+    StageTimer tm(p, s);
+    int rc = run_pre(p, in_u8, s, tm);
+    if (rc != FDD_OK) return rc;
+    return run_post(p, out, mode, s, tm, [](int, int) {});
+}
+
+int fdd_rotate_sum_only(fdd_plan* p, void* out, int mode, void* cuda_stream)
+{
+    if (check_plan(p) != FDD_OK || !out || (mode != FDD_MODE_TIME && mode != FDD_MODE_FOURIER))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    reset_profile(p);
+    StageTimer tm(p, s);
+    tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+    // FOURIER layout (pitch nbins) for either mode: `out` must hold ndm * nbins float2.
+    int rc = launch_rotate_sum(p, 0, p->ndm, static_cast<float2*>(out), p->nbins, mode, s);
+    tm.end();
+    return rc;
+}
+
+int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, int mode,
+                     void* cuda_stream)
+{
+    if (check_plan(p) != FDD_OK || !in_host || !out_host ||
+        (mode != FDD_MODE_TIME && mode != FDD_MODE_FOURIER))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t in_bytes = (size_t)p->nsamps * p->nchans;
+    const size_t row_bytes = mode == FDD_MODE_TIME ? (size_t)p->nsamps * sizeof(float)
+                                                   : (size_t)p->nbins * sizeof(float2);
+    const size_t out_bytes = row_bytes * p->ndm;
+    int rc;
+    if (!p->stage_in && (rc = dev_alloc(p, &p->stage_in, in_bytes)) != FDD_OK) return rc;
+    if (p->stage_out_bytes < out_bytes) {
+        if (p->stage_out) { cudaFree(p->stage_out); p->scratch_bytes -= p->stage_out_bytes; p->stage_out = nullptr; }
+        p->stage_out_bytes = 0;
+        if ((rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->stage_out), out_bytes)) != FDD_OK)
+            return rc;
+        p->stage_out_bytes = out_bytes;
+    }
+    if (!p->copy_stream &&
+        cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess)
+        return FDD_ERR_CUDA;
+    if (cudaMemcpyAsync(p->stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return FDD_ERR_CUDA;
+    reset_profile(p);
+    StageTimer tm(p, s);
+    rc = run_pre(p, p->stage_in, s, tm);
+    if (rc != FDD_OK) return rc;
+    size_t ev_used = 0;
+    bool copy_fail = false;
+    // Algorithm 1 lines 19-22: copy each finished DM chunk back while later chunks still compute.
+    auto chunk_done = [&](int j0, int rows) {
+        if (ev_used == p->chunk_events.size()) {
+            cudaEvent_t e;
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { copy_fail = true; return; }
+            p->chunk_events.push_back(e);
+        }
+        cudaEvent_t e = p->chunk_events[ev_used++];
+        if (cudaEventRecord(e, s) != cudaSuccess || cudaStreamWaitEvent(p->copy_stream, e, 0) != cudaSuccess ||
+            cudaMemcpyAsync(static_cast<char*>(out_host) + (size_t)j0 * row_bytes,
+                            static_cast<char*>(p->stage_out) + (size_t)j0 * row_bytes,
+                            (size_t)rows * row_bytes, cudaMemcpyDeviceToHost,
+                            p->copy_stream) != cudaSuccess)
+            copy_fail = true;
+    };
+    rc = run_post(p, p->stage_out, mode, s, tm, chunk_done);
+    if (rc != FDD_OK) return rc;
+    if (copy_fail) { cudaGetLastError(); return FDD_ERR_CUDA; }
+    if (cudaStreamSynchronize(p->copy_stream) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_CUDA;
+    }
+    return FDD_OK;
+}
+
+int fdd_plan_destroy(fdd_plan* p)
+{
+    destroy_plan(p);
+    return FDD_OK;
+}
+
+int fdd_plan_get_info(const fdd_plan* p, long long* nfft, long long* nbins, long long* valid_len,
+                      double* max_delay_samples, size_t* scratch_bytes, int* kernel)
+{
+    if (!p) return FDD_ERR_INVALID_ARG;
+    if (nfft) *nfft = p->nfft;
+    if (nbins) *nbins = p->nbins;
+    if (valid_len) *valid_len = p->valid_len;
+    if (max_delay_samples) *max_delay_samples = p->max_delay;
+    if (scratch_bytes) *scratch_bytes = p->scratch_bytes;
+    if (kernel) *kernel = p->kernel;
+    return FDD_OK;
+}
+
+int fdd_plan_get_delays(const fdd_plan* p, double* delay_samples_host)
+{
+    if (!p || !delay_samples_host) return FDD_ERR_INVALID_ARG;
+    memcpy(delay_samples_host, p->delays.data(), p->delays.size() * sizeof(double));
+    return FDD_OK;
+}
+
+int fdd_plan_set_profiling(fdd_plan* p, int enable)
+{
+    if (!p) return FDD_ERR_INVALID_ARG;
+    p->profiling = enable != 0;
+    return FDD_OK;
+}
+
+int fdd_plan_get_stage_ms(fdd_plan* p, float* ms_host, int* launches_host)
+{
+    if (!p || !ms_host) return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    for (int i = 0; i < FDD_NUM_STAGES; ++i) ms_host[i] = 0.f;
+    for (size_t i = 0; i < p->events_used; ++i) {
+        StageEvent& e = p->events[i];
+        if (cudaEventSynchronize(e.end) != cudaSuccess) { cudaGetLastError(); return FDD_ERR_CUDA; }
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.beg, e.end) != cudaSuccess) { cudaGetLastError(); return FDD_ERR_CUDA; }
+        ms_host[e.stage] += ms;
+    }
+    if (launches_host)
+        for (int i = 0; i < FDD_NUM_STAGES; ++i) launches_host[i] = p->launches[i];
+    return FDD_OK;
+}
+
+int fdd_plan_get_spectrum(const fdd_plan* p, void** x_dev, long long* pitch_elems)
+{
+    if (!p || !x_dev || !pitch_elems) return FDD_ERR_INVALID_ARG;
+    *x_dev = p->X;
+    *pitch_elems = p->xpitch;
+    return FDD_OK;
+}
+
+int fdd_measure_fp32_peak(int packed, int iters, double* tflops_host, float* ms_host)
+{
+    if (iters < 1 || !tflops_host) return FDD_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_CUDA;
+    }
+    float* sink = nullptr;
+    cudaEvent_t a = nullptr, b = nullptr;
+    int rc = FDD_ERR_CUDA;
+    const int blocks = sms * 8, threads = 256;
+    float ms = 0.f;
+    if (cudaMalloc(&sink, sizeof(float)) != cudaSuccess) { cudaGetLastError(); return FDD_ERR_ALLOC; }
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) goto done;
+    for (int rep = 0; rep < 2; ++rep) {          // first launch warms up
+        cudaEventRecord(a, 0);
+        if (packed) fdd::k_fp32_peak<true><<<blocks, threads>>>(sink, iters, 0.999f, 1e-3f);
+        else fdd::k_fp32_peak<false><<<blocks, threads>>>(sink, iters, 0.999f, 1e-3f);
+        cudaEventRecord(b, 0);
+        if (cudaEventSynchronize(b) != cudaSuccess) goto done;
+        cudaEventElapsedTime(&ms, a, b);
+    }
+    if (cudaGetLastError() != cudaSuccess) goto done;
+    // per thread per iteration: 4 unrolls * 8 chains * 2 lanes FMA = 64 FMA = 128 flop
+    *tflops_host = (double)blocks * threads * (double)iters * 128.0 / (ms * 1e-3) * 1e-12;
+    if (ms_host) *ms_host = ms;
+    rc = FDD_OK;
+done:
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(sink);
+    cudaGetLastError();
+    return rc;
+}
+
+const char* fdd_error_string(int status)
+{
+    switch (status) {
+        case FDD_OK: return "ok";
+        case FDD_ERR_INVALID_ARG: return "invalid argument";
+        case FDD_ERR_ALLOC: return "out of memory";
+        case FDD_ERR_CUDA: return "CUDA error";
+        case FDD_ERR_CUFFT: return "cuFFT error";
+        case FDD_ERR_UNSUPPORTED: return "unsupported";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

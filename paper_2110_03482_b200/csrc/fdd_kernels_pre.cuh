@@ -1,0 +1,102 @@
+// Step a2 (unpack + transpose + zero pad) and the FP32-rate probe.
+// Hand-written for sm_100a; HBM-bound.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fdd {
+
+// ---------------------------------------------------------------------------------------
+// a2: in  uint8 [nsamps][nchans] (channel fastest)
+//     out float [nchans][rpitch], out[c][t] = in[t][c] for t < nsamps, 0 for nsamps <= t < nfft
+// "transposed and unpacked ... in one kernel, thus requiring only a single pass",
+// "zero padded such that the number of samples becomes a power of two".
+// One CTA moves a 64 (time) x 64 (channel) tile through shared memory so that both the byte
+// reads (64 B runs along channels) and the float writes (128 B runs along time) are coalesced.
+// ---------------------------------------------------------------------------------------
+constexpr int kUnpackTile = 64;
+
+template <int VEC>
+__global__ void __launch_bounds__(256)
+k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int nchans,
+                   long long nsamps, long long nfft, long long rpitch)
+{
+    __shared__ float tile[kUnpackTile][kUnpackTile + 1];
+    const int tid = threadIdx.x;
+    const long long t0 = (long long)blockIdx.x * kUnpackTile;
+    const int c0 = blockIdx.y * kUnpackTile;
+
+    if (VEC == 4) {
+        const int trow = tid >> 4;          // 0..15
+        const int cq = (tid & 15) << 2;     // 0,4,..,60
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int tr = trow + 16 * i;
+            const long long t = t0 + tr;
+            uchar4 v = make_uchar4(0, 0, 0, 0);
+            if (t < nsamps && c0 + cq < nchans)
+                v = *reinterpret_cast<const uchar4*>(in + t * nchans + c0 + cq);
+            tile[cq + 0][tr] = (float)v.x;
+            tile[cq + 1][tr] = (float)v.y;
+            tile[cq + 2][tr] = (float)v.z;
+            tile[cq + 3][tr] = (float)v.w;
+        }
+    } else {
+        const int trow = tid >> 6;          // 0..3
+        const int cc = tid & 63;
+#pragma unroll 4
+        for (int i = 0; i < 16; ++i) {
+            const int tr = trow + 4 * i;
+            const long long t = t0 + tr;
+            float v = 0.f;
+            if (t < nsamps && c0 + cc < nchans) v = (float)in[t * nchans + c0 + cc];
+            tile[cc][tr] = v;
+        }
+    }
+    __syncthreads();
+    const int warp = tid >> 5, lane = tid & 31;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int cl = warp + 8 * i;
+        const int c = c0 + cl;
+        if (c >= nchans) continue;
+        float* row = out + (long long)c * rpitch;
+        const long long ta = t0 + lane, tb = t0 + 32 + lane;
+        if (ta < nfft) row[ta] = tile[cl][lane];
+        if (tb < nfft) row[tb] = tile[cl][lane + 32];
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// FP32 FMA-rate probe: register-resident dependent chains, 8 independent chains per thread.
+// packed = fma.rn.f32x2 (SASS FFMA2, two lanes per instruction), else scalar FFMA.
+// ---------------------------------------------------------------------------------------
+template <bool PACKED>
+__global__ void __launch_bounds__(256)
+k_fp32_peak(float* __restrict__ sink, int iters, float a, float b)
+{
+    float2 v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = make_float2(threadIdx.x * 1e-3f + i, blockIdx.x * 1e-3f - i);
+    const float2 aa = make_float2(a, a), bb = make_float2(b, b);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (PACKED) {
+                    v[i] = __ffma2_rn(v[i], aa, bb);
+                } else {
+                    v[i].x = fmaf(v[i].x, a, b);
+                    v[i].y = fmaf(v[i].y, a, b);
+                }
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += v[i].x + v[i].y;
+    if (s == 123.456f) sink[0] = s;   // never true in practice; keeps the chains alive
+}
+
+}  // namespace fdd

@@ -1,0 +1,299 @@
+"""GPU parity: the CUDA path through the C ABI against the CPU oracle, element by element.
+
+Tolerances are those of BASELINE.json north_star under the strict (mean-subtracted) reading,
+see tests/parity.py.  Integer work (the unpack stage, integer-delay shift-and-sum rounded to
+integers) is compared exactly.  Inputs are seeded and synthetic (synth/filterbank.py).
+"""
+import numpy as np
+import pytest
+
+import parity
+import synth
+from oracle import fdd_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def F():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2110_03482_b200 import build as fbuild
+    fbuild.build()
+    import paper_2110_03482_b200 as pkg
+    pkg.load_library()
+    return pkg
+
+
+def _run(F, plan, u8, mode):
+    import torch
+    d_in = torch.from_numpy(u8).cuda()
+    if mode == "time":
+        out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+    out = torch.empty((plan.ndm, plan.nbins, 2), dtype=torch.float32, device="cuda")
+    plan.execute(d_in, out, F.FDD_MODE_FOURIER)
+    torch.cuda.synchronize()
+    o = out.cpu().numpy()
+    return o[..., 0] + 1j * o[..., 1]
+
+
+def _plan_for(F, w):
+    return F.Plan.create(w.nchans, w.nsamps, w.tsamp, w.f_lo, w.f_hi, w.dm_list)
+
+
+def _delays_for(w):
+    return O.delay_table(w.nchans, w.f_lo, w.f_hi, w.tsamp, w.dm_list)
+
+
+KERNELS = ["generic", "auto"]
+
+
+def _set_kernel(F, plan, which):
+    plan.set_kernel(F.FDD_KERNEL_GENERIC if which == "generic" else F.FDD_KERNEL_AUTO)
+
+
+# ------------------------------------------------------------------ stages a2 + a3
+@pytest.mark.parametrize("nchans,nsamps", [(64, 8192), (7, 1000), (1, 64), (130, 4100)])
+def test_unpack_and_r2c_against_fp64_rfft(F, nchans, nsamps):
+    import torch
+    u8 = np.random.default_rng(nchans * 7 + nsamps).integers(0, 256, (nsamps, nchans), dtype=np.uint8)
+    with F.Plan.create(nchans, nsamps, 64e-6, 1200.0, 1500.0, [0.0]) as plan:
+        d_in = torch.from_numpy(u8).cuda()
+        out = torch.empty((1, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        ptr, pitch = plan.get_spectrum()
+        assert plan.nfft == O.next_pow2(nsamps) and plan.nbins == plan.nfft // 2 + 1
+        # view the plan's X in place through the CUDA array interface
+        class _View:
+            __cuda_array_interface__ = {"shape": (nchans, pitch, 2), "typestr": "<f4",
+                                        "data": (ptr, False), "version": 2}
+        xs = torch.as_tensor(_View(), device="cuda")
+        X = xs.cpu().numpy()
+        X = (X[..., 0] + 1j * X[..., 1])[:, :plan.nbins]
+        ref = np.fft.rfft(O.unpack(u8, plan.nfft), axis=-1)
+        # fp32 FFT of u8 data: error relative to the rms of the non-DC bins
+        rms = np.sqrt((np.abs(ref[:, 1:]) ** 2).mean())
+        assert np.abs(X - ref)[:, 1:].max() <= 2e-5 * rms * np.sqrt(np.log2(plan.nfft))
+        assert np.abs(X[:, 0] - ref[:, 0]).max() <= 1e-6 * np.abs(ref[:, 0]).max()
+        # DM = 0 output is the plain channel sum: integers, exact after rounding (a2 is exact)
+        y = out.cpu().numpy()[0]
+        assert np.array_equal(np.rint(y).astype(np.int64), u8.astype(np.int64).sum(axis=1))
+
+
+# ------------------------------------------------------------------ config 1, whole path
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("mode", ["time", "fourier"])
+def test_tiny_all_rows_against_naive_oracle(F, mode, kernel):
+    w = synth.workload("tiny")
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    ref = O.fdd_naive(u8, d, mode=mode)
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        nfft, nbins, valid, maxd, scratch, k = plan.get_info()
+        assert (nfft, nbins, valid) == (8192, 4097, 7927) and abs(maxd - d.max()) < 1e-9
+        assert np.abs(plan.get_delays() - d).max() <= 1e-9
+        got = _run(F, plan, u8, mode)
+    worst = parity.assert_rows(got, ref, mode, f"tiny/{mode}/{kernel}")
+    print("tiny", mode, kernel, worst)
+    if mode == "time":
+        peak = got.max(axis=1)
+        assert int(np.argmax(peak)) == 15 and abs(int(np.argmax(got[15])) - 2048) <= 1
+
+
+# ------------------------------------------------------------------ ragged / edge shapes
+RAGGED = [
+    # nchans, nsamps, ndm, dm_step, dm0
+    (5, 1000, 3, 7.5, 0.0),          # zero padding 1000 -> 1024, odd channel count
+    (1, 256, 4, 10.0, 0.0),          # single channel: all delays zero
+    (64, 2048, 1, 3.0, 12.0),        # single DM
+    (33, 4096, 37, 1.25, -5.0),      # negative DMs, ndm ragged against every tile size
+    (96, 6000, 70, 0.9, 3.3),        # padded 6000 -> 8192, two DM tiles + tail
+    (2, 2, 2, 1.0, 0.0),             # smallest legal nsamps
+]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("mode", ["time", "fourier"])
+@pytest.mark.parametrize("nchans,nsamps,ndm,step,dm0", RAGGED)
+def test_ragged_shapes(F, nchans, nsamps, ndm, step, dm0, mode, kernel):
+    w = synth.small_workload(100 + nchans, nchans, nsamps, ndm, dm_step=step, dm0=dm0, mode=mode)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    ref = O.fdd_fft(u8, d, mode=mode)
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        got = _run(F, plan, u8, mode)
+        assert plan.get_info()[2] == O.valid_length(d, nsamps)
+    if nsamps >= 256:
+        parity.assert_rows(got, ref, mode, f"ragged {nchans}x{nsamps}x{ndm}/{mode}/{kernel}")
+    else:
+        scale = np.abs(ref).max()
+        assert np.abs(got - ref).max() <= 1e-5 * scale
+
+
+def test_non_uniform_dm_list_and_kdm_override(F):
+    rng = np.random.default_rng(5)
+    dms = np.sort(rng.uniform(0, 300, size=45))
+    dms[7] = dms[6]                                      # duplicate (S20)
+    w = synth.small_workload(77, 48, 4096, 2)
+    u8 = synth.make_filterbank(w)
+    kdm = 1.0 / 2.41e-4                                  # the paper's constant
+    d = O.delay_table(48, w.f_lo, w.f_hi, w.tsamp, dms, k_dm=kdm)
+    ref = O.fdd_fft(u8, d)
+    with F.Plan.create(48, 4096, w.tsamp, w.f_lo, w.f_hi, dms) as plan:
+        plan.set_kdm(kdm)
+        assert np.abs(plan.get_delays() - d).max() <= 1e-9
+        got = _run(F, plan, u8, "time")
+    parity.assert_rows(got, ref, "time", "non-uniform DM list")
+
+
+# ------------------------------------------------------------------ P3 on the GPU: exact integers
+def _integer_reference(u8, d, rows):
+    ref = np.zeros((len(rows), u8.shape[0]), dtype=np.int64)
+    for i, j in enumerate(rows):
+        for c in range(u8.shape[1]):
+            ref[i] += np.roll(u8[:, c].astype(np.int64), -int(d[j, c]))
+    return ref
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_integer_delays_equal_circular_shift_and_sum(F, kernel):
+    nchans, nsamps, ndm = 128, 1 << 14, 40
+    u8 = np.random.default_rng(9).integers(0, 256, (nsamps, nchans), dtype=np.uint8)
+    d = synth.integer_delay_table(11, ndm, nchans, 3000)
+    ref = _integer_reference(u8, d, range(ndm))
+    with F.Plan.create_from_delays(nchans, nsamps, d) as plan:
+        _set_kernel(F, plan, kernel)
+        got = _run(F, plan, u8, "time")
+    # integer sums of 128 bytes (<= 32640): fp32 path must land within 0.02 of the integer
+    assert np.abs(got - ref).max() <= 0.05
+    assert np.array_equal(np.rint(got).astype(np.int64), ref)
+    parity.assert_rows(got, ref.astype(np.float64), "time", "integer delays")
+
+
+# ------------------------------------------------------------------ host-buffer entry point
+def test_execute_host_matches_execute(F):
+    import torch
+    w = synth.small_workload(31, 64, 8192, 48)
+    u8 = synth.make_filterbank(w)
+    with _plan_for(F, w) as plan:
+        dev = _run(F, plan, u8, "time")
+        h_in = torch.from_numpy(u8).pin_memory()
+        h_out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32).pin_memory()
+        plan.execute_host(h_in, h_out, F.FDD_MODE_TIME)
+        assert np.array_equal(h_out.numpy(), dev)
+        h_outf = torch.empty((plan.ndm, plan.nbins, 2), dtype=torch.float32)      # pageable
+        plan.execute_host(u8, h_outf, F.FDD_MODE_FOURIER)
+        devf = _run(F, plan, u8, "fourier")
+        assert np.array_equal(h_outf.numpy()[..., 0] + 1j * h_outf.numpy()[..., 1], devf)
+
+
+def test_stage_profile_and_errors(F):
+    import torch
+    w = synth.small_workload(32, 16, 1024, 8)
+    u8 = synth.make_filterbank(w)
+    with _plan_for(F, w) as plan:
+        plan.set_profiling(True)
+        _run(F, plan, u8, "time")
+        ms, launches = plan.get_stage_ms()
+        assert all(v >= 0 for v in ms.values()) and ms["rotate_sum"] > 0
+        assert launches["unpack"] == 1 and launches["r2c"] == 1 and launches["rotate_sum"] >= 1
+        with pytest.raises(F.FddError):
+            plan.execute(torch.zeros(4, device="cuda"), 0, F.FDD_MODE_TIME)     # NULL out
+        with pytest.raises(F.FddError):
+            plan.execute(torch.zeros(4, device="cuda"), torch.zeros(4, device="cuda"), 7)
+    tf, ms_ = F.measure_fp32_peak(True, 256)
+    assert tf > 1.0
+
+
+# ------------------------------------------------------------------ full-size configs (sampled rows)
+def _sampled_rows(ndm, n, seed):
+    rng = np.random.default_rng(seed)
+    rows = {0, ndm - 1}
+    while len(rows) < min(n, ndm):
+        rows.add(int(rng.integers(0, ndm)))
+    return sorted(rows)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,nrows", [("config2", 16), ("config3", 8)])
+def test_full_size_time_configs(F, oracle_c, name, nrows):
+    import torch
+    w = synth.workload(name)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = _sampled_rows(w.ndm, nrows, w.seed)
+    ref = O.fdd_rows(u8, d, rows, mode="time")
+    with _plan_for(F, w) as plan:
+        assert plan.get_info()[2] == w.nsamps - (w.ndm - 1)
+        d_in = torch.from_numpy(u8).cuda()
+        out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        got = out[rows].cpu().numpy()
+        # properties that hold at any size: DM 0 is the exact channel sum; DC invariance (P7)
+        y0 = out[0].cpu().numpy()
+        assert np.array_equal(np.rint(y0).astype(np.int64), u8.astype(np.int64).sum(axis=1))
+        total = float(u8.astype(np.int64).sum())
+        sums = out.double().sum(dim=1).cpu().numpy()
+        assert np.abs(sums - total).max() <= 2e-6 * total
+    worst = parity.assert_rows(got, ref, "time", name)
+    print(name, "rows", rows, worst)
+
+
+@pytest.mark.slow
+def test_full_size_config5_fourier(F, oracle_c):
+    import torch
+    w = synth.workload("config5")
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = _sampled_rows(w.ndm, 6, w.seed) + [2680]           # DM 26.8 = trial 2680
+    rows = sorted(set(rows))
+    ref = O.fdd_rows(u8, d, rows, mode="fourier")
+    bins = sorted(set(np.random.default_rng(55).integers(1, w.nsamps // 2, 62).tolist()
+                      + [1, w.nsamps // 2]))
+    ref_bins = O.single_bins(u8, d, bins, rows=rows)            # straight from the definition
+    with _plan_for(F, w) as plan:
+        d_in = torch.from_numpy(u8).cuda()
+        out = torch.empty((plan.ndm, plan.nbins, 2), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_FOURIER)
+        torch.cuda.synchronize()
+        o = out[rows].cpu().numpy()
+        got = o[..., 0] + 1j * o[..., 1]
+        power = (out[:, 1:, 0].double() ** 2 + out[:, 1:, 1].double() ** 2)
+        # the periodic pulse train (P = 0.714 s, fundamental near bin 360.9) is brightest at DM 26.8
+        harm = [int(round(h * w.nsamps * w.tsamp / 0.714)) - 1 for h in range(1, 9)]
+        hp = power[:, harm].sum(dim=1).cpu().numpy()
+        assert abs(int(np.argmax(hp)) - 2680) <= 3
+    worst = parity.assert_rows(got, ref, "fourier", "config5")
+    print("config5 rows", rows, worst)
+    rms = np.sqrt((np.abs(ref[:, 1:]) ** 2).mean())
+    assert np.abs(got[:, bins] - ref_bins).max() <= 1e-3 * rms
+    assert np.abs(ref[:, bins] - ref_bins).max() <= 1e-9 * rms     # P10 at full size
+
+
+@pytest.mark.slow
+def test_full_size_integer_delays(F):
+    """P3 at 1024 channels x 2^20 samples: no FFT anywhere in the reference."""
+    import torch
+    nchans, nsamps, ndm = 1024, 1 << 20, 64
+    w = synth.workload("config3")
+    u8 = synth.make_filterbank(w)
+    d = synth.integer_delay_table(13, ndm, nchans, 1023)
+    rows = [0, 1, 17, 31, 32, 40, 62, 63]
+    ref = _integer_reference(u8, d, rows)
+    with F.Plan.create_from_delays(nchans, nsamps, d) as plan:
+        d_in = torch.from_numpy(u8).cuda()
+        out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        got = out[rows].cpu().numpy()
+    parity.assert_rows(got, ref.astype(np.float64), "time", "integer delays, full size")
+    # sums of 1024 bytes reach 1.3e5 where the fp32 ulp is 1/64: the rounded value is the integer
+    assert np.abs(got - ref).max() <= 0.25
+    assert np.array_equal(np.rint(got).astype(np.int64), ref)
