@@ -1,0 +1,400 @@
+#!/usr/bin/env python
+"""bench.py -- dedispersion rate of the FDD hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--ndm D] [--impl reference]
+
+A step is one pass of the whole hot path (a2 unpack+transpose, a3 R2C, a4 phase-rotate-and-sum,
+a5 C2R) over one seeded synthetic filterbank (synth/filterbank.py).  Default workload: the
+configuration BASELINE.json's target is quoted on, config 4 at 4096 trial DMs (1024 channels x
+2^20 samples), which fits one GPU.  metric = DM-trials x samples / s.
+
+  value      K steps through fdd_execute with the input resident in HBM, CUDA events on the
+             launching stream, barrier + synchronize on both sides, max over ranks
+  e2e        the same metric through fdd_execute_host: pinned HOST input and output, both
+             copies inside the timed region
+  roofline   the dominant kernel (a4): algorithmic 8 flop per (dm, channel, bin) element over
+             its mean launch duration (CUDA events recorded by the library between the stages,
+             inside the timed region), against the FP32 FMA rate measured live on the same GPU
+             by a register-resident FFMA2 loop
+  cpu_baseline  the CPU oracle as it stands, timed on the host cores on a bounded sample
+
+N > 1 (torchrun): weak scaling by trial-DM range -- every rank dedisperses the same input over
+its own block of ndm trial DMs (rank r: trials r*ndm .. (r+1)*ndm - 1); no data-path collective
+(DESIGN.md "Multi-GPU").  --impl reference times the oracle (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "dedispersion_rate"
+UNIT = "DM-trials*samples/s"
+FLOP_PER_ELEMENT = 8.0          # one complex MAC per (dm, channel, bin): SURVEY.md 8d
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="config4",
+                    choices=["tiny", "config2", "config3", "config4", "config5"])
+    ap.add_argument("--ndm", type=int, default=None, help="trial DMs (config 4 sweep point)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "symmetric"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-rows", type=int, default=3, help="DM rows the oracle sample computes")
+    return ap.parse_args()
+
+
+def dist_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+def make_workload(args, rank: int, world: int):
+    """The synthetic workload of this rank: rank r takes trial DMs [r*ndm, (r+1)*ndm)."""
+    import synth
+    w = synth.workload(args.workload, ndm=args.ndm)
+    ndm = w.ndm
+    if world > 1:
+        step = w.dm_list[1] - w.dm_list[0] if ndm > 1 else 0.0
+        dms = tuple(w.dm_list[0] + step * (rank * ndm + i) for i in range(ndm))
+        import dataclasses
+        w = dataclasses.replace(w, dm_list=dms)
+    return w
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {
+        0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+        0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+        0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thread = None
+        self.period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._stop.clear()
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join()
+            self._thread = None
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0}
+        reasons = [n for b, n in self.REASONS.items() if self.reason_bits & b and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.sm_max,
+                "reasons": reasons, "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(w, u8, nrows: int, cfft: int = 256):
+    """Time the oracle (oracle/, as it stands) on a bounded sample of workload ``w``.
+
+    The oracle's cost is  t_fft (O1+O2, once per input)  +  rows * t_row (O4+O5 per trial DM),
+    exactly linear in the rows; both parts are measured on this box and the whole-workload time
+    is t_fft + ndm * t_row.  Returns (rate, description, threads, seconds spent).
+    """
+    from oracle import build as obuild
+    obuild.build()
+    from oracle import fdd_oracle as O
+    t_start = time.time()
+    d = O.delay_table(w.nchans, w.f_lo, w.f_hi, w.tsamp, w.dm_list)
+    n = O.next_pow2(w.nsamps)
+    rng = np.random.default_rng(w.seed)
+    rows = sorted({0, w.ndm - 1} | set(int(r) for r in rng.integers(0, w.ndm, max(nrows - 2, 0))))
+    rows = rows[:max(nrows, 1)]
+    # O1+O2 on a bounded subset of channels (cost is linear in channels), scaled to all of them
+    cfft = min(w.nchans, cfft)
+    t0 = time.time()
+    X = np.fft.rfft(O.unpack(u8[:, :cfft], n), axis=-1)
+    t_fft = (time.time() - t0) * (w.nchans / cfft)
+    # O4 for the sampled rows over a bounded channel subset, scaled; O5 per row
+    t0 = time.time()
+    Y = O.phase_rotate_sum_c(X, d[rows][:, :cfft], n)
+    t_o4 = (time.time() - t0) * (w.nchans / cfft) / len(rows)
+    t_o5 = 0.0
+    if w.mode == "time":
+        t0 = time.time()
+        np.fft.irfft(Y, n=n, axis=-1)
+        t_o5 = (time.time() - t0) / len(rows)
+    t_full = t_fft + w.ndm * (t_o4 + t_o5)
+    rate = w.ndm * w.nsamps / t_full
+    what = (f"{len(rows)} of {w.ndm} DM rows x {cfft} of {w.nchans} channels x all {w.nsamps} samples "
+            f"(fp64 FFT {t_fft:.1f} s per input + {t_o4 + t_o5:.2f} s per DM row, both linear, "
+            f"scaled to the whole workload: {t_full:.0f} s)")
+    return rate, what, O.num_threads(), time.time() - t_start
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the oracle timed on the host cores, rank 0 only."""
+    if rank != 0:
+        return
+    import synth
+    w = make_workload(args, 0, 1)
+    u8 = synth.make_filterbank(w)
+    budget = 150.0 / max(args.steps + args.warmup, 1)        # seconds of CPU work per step
+    rates, what, threads = [], "", 1
+    nrows, cfft = 2, 256
+    for it in range(args.warmup + args.steps):
+        rate, what, threads, spent = oracle_sample(w, u8, nrows, cfft)
+        if it >= args.warmup:
+            rates.append(rate)
+        if spent > budget and cfft > 16:
+            cfft //= 2
+    value = float(np.mean(rates))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * w.ndm * w.nsamps / value, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, world: int):
+    return {"workload": f"{w.name}: {w.nchans} channels {w.f_lo:g}-{w.f_hi:g} MHz, "
+                        f"{w.nsamps} samples of {w.tsamp * 1e6:g} us, {w.ndm} trial DMs per GPU, "
+                        f"{w.mode}-domain output",
+            "nchans": w.nchans, "nsamps": w.nsamps, "ndm_per_gpu": w.ndm, "ndm_total": w.ndm * world,
+            "mode": w.mode, "seed": w.seed,
+            "l2": "inputs larger than L2 (no flush needed): u8 input, X and Y are each >= 1 GiB"
+                  if w.nsamps * w.nchans > (1 << 28) else "L2 flushed between steps"}
+
+
+# ----------------------------------------------------------------------------- the CUDA arm
+def run_b200(args, rank: int, local_rank: int, world: int):
+    import torch
+    import torch.distributed as dist
+    import synth
+    from paper_2110_03482_b200 import build as fbuild
+    if rank == 0:
+        fbuild.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the FDD path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    import paper_2110_03482_b200 as F
+    F.load_library()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args, rank, world)
+    u8 = synth.make_filterbank(w)                       # same bytes on every rank (same seed)
+    mode = F.FDD_MODE_TIME if w.mode == "time" else F.FDD_MODE_FOURIER
+    plan = F.Plan.create(w.nchans, w.nsamps, w.tsamp, w.f_lo, w.f_hi, w.dm_list)
+    plan.set_kernel({"auto": F.FDD_KERNEL_AUTO, "generic": F.FDD_KERNEL_GENERIC,
+                     "symmetric": F.FDD_KERNEL_SYMMETRIC}[args.kernel])
+    nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
+    d_in = torch.from_numpy(u8).cuda()
+    if mode == F.FDD_MODE_TIME:
+        out = torch.empty((w.ndm, w.nsamps), dtype=torch.float32, device="cuda")
+    else:
+        out = torch.empty((w.ndm, nbins, 2), dtype=torch.float32, device="cuda")
+    flush = None
+    if w.nsamps * w.nchans <= (1 << 28):
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        if flush is not None:
+            flush.fill_(1)
+        plan.execute(d_in, out, mode, stream)
+
+    # FP32 FMA rate of this GPU, measured with the library's FFMA2 probe (~0.25 s, sustained)
+    peak_tf, peak_ms = F.measure_fp32_peak(True, 1 << 19)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ
+                           else int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+    plan.set_profiling(True)                              # zeroes the stage totals
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    stage_ms, launches = plan.get_stage_ms()
+    plan.set_profiling(False)
+    if flush is not None:                                  # the flush is not part of the path
+        ms_total = sum(stage_ms.values())
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    units = float(w.ndm) * w.nsamps * world               # DM-trials x samples, all ranks
+    value = units / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point ---------------------------------
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.from_numpy(u8).pin_memory()
+        h_out = torch.empty(out.shape, dtype=torch.float32, pin_memory=True)
+        plan.execute_host(h_in, h_out, mode, stream)       # warm-up: staging buffers, page faults
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            plan.execute_host(h_in, h_out, mode, stream)   # returns when the result is on the host
+        barrier()
+        t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        e2e = {"value": units / (float(t_e2e.item()) / args.e2e_steps), "unit": UNIT,
+               "h2d_bytes_per_step": int(h_in.numel()) * world,
+               "d2h_bytes_per_step": int(h_out.numel()) * 4 * world,
+               "steps": args.e2e_steps, "host_memory": "pinned",
+               "timer": "host perf_counter around fdd_execute_host (synchronous), max over ranks"}
+        del h_in, h_out
+
+    if rank != 0:
+        plan.destroy()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (a4) ---------------------------------------------
+    elements = float(w.ndm) * w.nchans * nbins
+    sum_ms = stage_ms["rotate_sum"] / args.steps
+    achieved = FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tpath):
+        try:
+            tj = json.load(open(tpath))
+            key = f"{w.name}/{w.ndm}/kernel{kernel}"
+            traffic = tj.get(key)
+        except Exception:
+            traffic = None
+    roofline = {
+        "kernel": "k_rotate_sum_sym" if kernel == F.FDD_KERNEL_SYMMETRIC else "k_rotate_sum_generic",
+        "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+        "frac": achieved / peak_tf, "traffic": traffic,
+        "peak_source": "measured live: fdd_measure_fp32_peak (FFMA2 register loop, all SMs, "
+                       f"{peak_ms:.0f} ms); cross-check 148 SM x 128 lanes x 2 x 1.965 GHz = 74.45",
+        "algorithmic": "8 flop (one complex MAC) per (dm, channel, bin) element; the symmetric "
+                       "kernel executes 6 FP32 lane-operations (3 FFMA2 lanes) per element",
+        "ms_per_launch": sum_ms, "share_of_step": sum_ms / ms_step,
+    }
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(w, world),
+        "clocks": sampler.summary(),
+        "e2e": e2e,
+        "gpu_launches": int((launches["unpack"] + launches["rotate_sum"])),
+        "library_calls": int(launches["r2c"] + launches["c2r"]),
+        "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+        "roofline": roofline,
+        "plan": {"nfft": nfft, "nbins": nbins, "valid_len": valid, "max_delay_samples": maxd,
+                 "scratch_bytes": scratch, "kernel": kernel},
+    }
+    # HBM-bound stages: achieved GB/s against the measured copy bandwidth
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    pitch = 2 * ((nbins + 15) // 16 * 16)
+    stage_bytes = {
+        "unpack": w.nchans * w.nsamps + 4.0 * w.nchans * nfft,
+        "r2c": 4.0 * w.nchans * nfft + 8.0 * w.nchans * nbins,
+        "c2r": (8.0 * w.ndm * nbins + 4.0 * w.ndm * nfft) if mode == F.FDD_MODE_TIME else 0.0,
+    }
+    line["hbm_stages"] = {
+        k: {"algorithmic_gb": b * 1e-9, "gbs": b * 1e-9 / (line["stage_ms_per_step"][k] * 1e-3),
+            "frac_of_copy_peak": b * 1e-9 / (line["stage_ms_per_step"][k] * 1e-3) / hbm}
+        for k, b in stage_bytes.items() if line["stage_ms_per_step"][k] > 0}
+    line["hbm_peak_gbs"] = hbm
+    line["hbm_peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback 6650 (B200_PROFILING.md)"
+
+    if world == 1 and not args.no_cpu_baseline:
+        plan.destroy()
+        del d_in, out
+        torch.cuda.empty_cache()
+        rate, what, threads, _ = oracle_sample(w, u8, args.cpu_rows)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": what, "host_cores": os.cpu_count()}
+    else:
+        plan.destroy()
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank, local_rank, world = dist_env()
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    run_b200(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

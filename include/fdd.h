@@ -135,10 +135,12 @@ int fdd_plan_get_info(const fdd_plan *plan, long long *nfft, long long *nbins,
 /* Copy the plan's delay table to delay_samples_host[ndm][nchans] (HOST). */
 int fdd_plan_get_delays(const fdd_plan *plan, double *delay_samples_host);
 
-/* Stage timing.  fdd_plan_set_profiling(plan, 1) makes fdd_execute record CUDA events between
- * the stages on its stream; fdd_plan_get_stage_ms then waits for the last execute and writes
- * the device time of each stage in milliseconds to ms_host[FDD_NUM_STAGES] (0 for a skipped
- * stage) and, if launches_host != NULL, how many kernels/library calls each stage launched. */
+/* Stage timing.  fdd_plan_set_profiling(plan, 1) makes every following execute record CUDA
+ * events between the stages on its stream, and zeroes the totals; fdd_plan_get_stage_ms waits
+ * for the last execute and writes the device time of each stage, summed over all executes since
+ * that call, in milliseconds to ms_host[FDD_NUM_STAGES] (0 for a skipped stage) and, if
+ * launches_host != NULL, how many kernels / library calls each stage launched in total (counted
+ * with profiling on or off). */
 int fdd_plan_set_profiling(fdd_plan *plan, int enable);
 int fdd_plan_get_stage_ms(fdd_plan *plan, float *ms_host, int *launches_host);
 

@@ -525,7 +525,6 @@ int fdd_execute(fdd_plan* p, const unsigned char* in_u8, void* out, int mode, vo
     DeviceGuard g(p->device);
     if (!g.ok) return FDD_ERR_CUDA;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    reset_profile(p);
     StageTimer tm(p, s);
     int rc = run_pre(p, in_u8, s, tm);
     if (rc != FDD_OK) return rc;
@@ -539,7 +538,6 @@ int fdd_rotate_sum_only(fdd_plan* p, void* out, int mode, void* cuda_stream)
     DeviceGuard g(p->device);
     if (!g.ok) return FDD_ERR_CUDA;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    reset_profile(p);
     StageTimer tm(p, s);
     tm.begin(FDD_STAGE_ROTATE_SUM, 1);
     // FOURIER layout (pitch nbins) for either mode: `out` must hold ndm * nbins float2.
@@ -575,7 +573,6 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
         return FDD_ERR_CUDA;
     if (cudaMemcpyAsync(p->stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
         return FDD_ERR_CUDA;
-    reset_profile(p);
     StageTimer tm(p, s);
     rc = run_pre(p, p->stage_in, s, tm);
     if (rc != FDD_OK) return rc;
@@ -636,6 +633,7 @@ int fdd_plan_set_profiling(fdd_plan* p, int enable)
 {
     if (!p) return FDD_ERR_INVALID_ARG;
     p->profiling = enable != 0;
+    reset_profile(p);
     return FDD_OK;
 }
 
