@@ -22,6 +22,7 @@ constexpr double kDefaultKdm = 4.148808e3;            // MHz^2 pc^-1 cm^3 s (DES
 constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
 constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
 constexpr int kC2RBatch = 256;                        // rows per cuFFT C2R call (bounds workspace)
+constexpr int kHostChunkRows = 2 * kC2RBatch;         // fdd_execute_host: DM rows per pipelined chunk
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
@@ -414,20 +415,29 @@ int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer&
 
 // Stages a4+a5 from the spectra in p->X.  chunk_done (optional) is called after each DM chunk
 // has been queued, with (j_begin, rows), so fdd_execute_host can overlap the copy back.
+// chunk_rows > 0 caps the DM rows per chunk (multiple of kC2RBatch), for copy/compute overlap.
 template <class F>
-int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F chunk_done)
+int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F chunk_done,
+             int chunk_rows = 0)
 {
     if (mode == FDD_MODE_FOURIER) {
-        tm.begin(FDD_STAGE_ROTATE_SUM, 1);
-        int rc = launch_rotate_sum(p, 0, p->ndm, static_cast<float2*>(out), p->nbins, mode, s);
-        tm.end();
-        if (rc == FDD_OK) chunk_done(0, p->ndm);
-        return rc;
+        const int step = chunk_rows > 0 ? chunk_rows : p->ndm;
+        for (int j0 = 0; j0 < p->ndm; j0 += step) {
+            const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
+            tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+            int rc = launch_rotate_sum(p, j0, rows, static_cast<float2*>(out) + (long long)j0 * p->nbins,
+                                       p->nbins, mode, s);
+            tm.end();
+            if (rc != FDD_OK) return rc;
+            chunk_done(j0, rows);
+        }
+        return FDD_OK;
     }
     int rc = ensure_time_resources(p);
     if (rc != FDD_OK) return rc;
-    for (int j0 = 0; j0 < p->ndm; j0 += p->y_rows) {
-        const int rows = (p->ndm - j0 < p->y_rows) ? p->ndm - j0 : p->y_rows;
+    const int step = (chunk_rows > 0 && chunk_rows < p->y_rows) ? chunk_rows : p->y_rows;
+    for (int j0 = 0; j0 < p->ndm; j0 += step) {
+        const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
         tm.begin(FDD_STAGE_ROTATE_SUM, 1);
         rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s);
         tm.end();
@@ -593,7 +603,8 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
                             p->copy_stream) != cudaSuccess)
             copy_fail = true;
     };
-    rc = run_post(p, p->stage_out, mode, s, tm, chunk_done);
+    // DM chunks of kHostChunkRows rows: the copy back of chunk i overlaps the compute of chunk i+1
+    rc = run_post(p, p->stage_out, mode, s, tm, chunk_done, kHostChunkRows);
     if (rc != FDD_OK) return rc;
     if (copy_fail) { cudaGetLastError(); return FDD_ERR_CUDA; }
     if (cudaStreamSynchronize(p->copy_stream) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
