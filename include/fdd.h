@@ -145,8 +145,13 @@ int fdd_plan_set_profiling(fdd_plan *plan, int enable);
 int fdd_plan_get_stage_ms(fdd_plan *plan, float *ms_host, int *launches_host);
 
 /* Debug/test access: DEVICE pointer to the channel spectra X (float2 [nchans][pitch]) left by
- * the last execute, and the row pitch in float2 elements. */
-int fdd_plan_get_spectrum(const fdd_plan *plan, void **x_dev, long long *pitch_elems);
+ * the last execute, and the row pitch in float2 elements.  When nsamps is a power of two the
+ * unpack step subtracts 128 from every sample (exact) so that the mean of unsigned-byte data
+ * stays out of the fp32 FFTs; the sum kernel restores it in bin 0.  *dc_removed (may be NULL)
+ * receives what has to be added to Re X[c][0] of every channel to get the plain DFT
+ * (128 * nsamps, or 0 when the input is zero padded). */
+int fdd_plan_get_spectrum(const fdd_plan *plan, void **x_dev, long long *pitch_elems,
+                          double *dc_removed);
 
 /* Run only a4 on the spectra left by the last execute (for timing sweeps of the hot kernel). */
 int fdd_rotate_sum_only(fdd_plan *plan, void *out, int mode, void *cuda_stream);

@@ -60,7 +60,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_get_delays.argtypes = [vp, P(c_dbl)]
     lib.fdd_plan_set_profiling.argtypes = [vp, c_int]
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
-    lib.fdd_plan_get_spectrum.argtypes = [vp, P(vp), P(c_ll)]
+    lib.fdd_plan_get_spectrum.argtypes = [vp, P(vp), P(c_ll), P(c_dbl)]
     lib.fdd_rotate_sum_only.argtypes = [vp, vp, c_int, vp]
     lib.fdd_measure_fp32_peak.argtypes = [c_int, c_int, P(c_dbl), P(ctypes.c_float)]
     for name in EXPORTS:
@@ -187,12 +187,12 @@ class Plan:
         return ({n: float(ms[i]) for i, n in enumerate(STAGE_NAMES)},
                 {n: int(ln[i]) for i, n in enumerate(STAGE_NAMES)})
 
-    def get_spectrum(self) -> Tuple[int, int]:
-        """(device pointer, row pitch in float2 elements) of X[nchans][pitch]."""
-        x, pitch = ctypes.c_void_p(), ctypes.c_longlong()
-        _check(load_library().fdd_plan_get_spectrum(self._h, ctypes.byref(x),
-                                                    ctypes.byref(pitch)), "fdd_plan_get_spectrum")
-        return x.value, pitch.value
+    def get_spectrum(self) -> Tuple[int, int, float]:
+        """(device pointer, row pitch in float2 elements, DC removed per channel) of X[nchans][pitch]."""
+        x, pitch, dc = ctypes.c_void_p(), ctypes.c_longlong(), ctypes.c_double()
+        _check(load_library().fdd_plan_get_spectrum(self._h, ctypes.byref(x), ctypes.byref(pitch),
+                                                    ctypes.byref(dc)), "fdd_plan_get_spectrum")
+        return x.value, pitch.value, dc.value
 
     def destroy(self) -> None:
         if self._h is not None and self._h.value:

@@ -44,6 +44,7 @@ struct fdd_plan {
     double max_delay = 0;
     long long valid_len = 0;
     int device = 0;
+    float offset = 0.f;                  // subtracted by a2, restored in bin 0 by a4 (S21)
     // device buffers
     float2* X = nullptr;                 // [nchans][xpitch]; also the real rows of the in-place R2C
     long long xpitch = 0;
@@ -279,6 +280,8 @@ int create_common(fdd_plan* p)
     p->nfft = 2;
     while (p->nfft < p->nsamps) p->nfft <<= 1;
     p->nbins = p->nfft / 2 + 1;
+    // Without zero padding a constant offset lives in bin 0 alone; with padding it would not.
+    p->offset = p->nsamps == p->nfft ? 128.f : 0.f;
     p->xpitch = round_up(p->nbins, kPitchAlign);
     p->ndm_pad = (int)round_up(p->ndm, fdd::kGenDT);
     int rc = dev_alloc(p, &p->X, (size_t)p->nchans * p->xpitch);
@@ -338,10 +341,10 @@ int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
     const bool vec = (p->nchans % 4 == 0) && ((uintptr_t)in_u8 % 4 == 0);
     if (vec)
         fdd::k_unpack_transpose<4><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        2 * p->xpitch);
+                                                        2 * p->xpitch, p->offset);
     else
         fdd::k_unpack_transpose<1><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        2 * p->xpitch);
+                                                        2 * p->xpitch, p->offset);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
@@ -351,15 +354,18 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
 {
     const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
     const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
+    // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
+    const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
+    const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
     if (p->kernel == FDD_KERNEL_SYMMETRIC)
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
-                               dst, opitch, scale, real_edges, s);
+                               dst, opitch, scale, real_edges, dc_add, s);
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
     const long long n_kt = (p->nbins + fdd::kGenThreads - 1) / fdd::kGenThreads;
     if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
     fdd::k_rotate_sum_generic<<<(unsigned)(n_jt * n_kt), fdd::kGenThreads, 0, s>>>(
         p->X, p->xpitch, p->phase64, p->ndm_pad, p->nchans, p->nbins, j_begin + rows, j_begin, n_jt,
-        dst, opitch, scale, real_edges);
+        dst, opitch, scale, real_edges, dc_add);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
@@ -665,11 +671,13 @@ int fdd_plan_get_stage_ms(fdd_plan* p, float* ms_host, int* launches_host)
     return FDD_OK;
 }
 
-int fdd_plan_get_spectrum(const fdd_plan* p, void** x_dev, long long* pitch_elems)
+int fdd_plan_get_spectrum(const fdd_plan* p, void** x_dev, long long* pitch_elems,
+                          double* dc_removed)
 {
     if (!p || !x_dev || !pitch_elems) return FDD_ERR_INVALID_ARG;
     *x_dev = p->X;
     *pitch_elems = p->xpitch;
+    if (dc_removed) *dc_removed = (double)p->offset * (double)p->nsamps;
     return FDD_OK;
 }
 

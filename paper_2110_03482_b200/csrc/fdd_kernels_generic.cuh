@@ -33,7 +33,8 @@ __global__ void __launch_bounds__(kGenThreads)
 k_rotate_sum_generic(const float2* __restrict__ X, long long xpitch,
                      const unsigned long long* __restrict__ phase64, int ndm_pad, int nchans,
                      long long nbins, int ndm, int j_begin, int n_jtiles,
-                     float2* __restrict__ out, long long opitch, float scale, int real_edges)
+                     float2* __restrict__ out, long long opitch, float scale, int real_edges,
+                     float dc_add)
 {
     // 1-D grid, DM tile fastest: CTAs resident together share X columns through L2.
     const int jt = blockIdx.x % n_jtiles;
@@ -67,7 +68,8 @@ k_rotate_sum_generic(const float2* __restrict__ X, long long xpitch,
     for (int i = 0; i < kGenDT; ++i) {
         const int j = j0 + i;
         if (j >= ndm) break;
-        float2 v = make_float2(acc[i].x * scale, edge ? 0.f : acc[i].y * scale);
+        float2 v = make_float2(acc[i].x * scale + (k == 0 ? dc_add : 0.f),
+                               edge ? 0.f : acc[i].y * scale);
         out[(long long)(j - j_begin) * opitch + k] = v;
     }
 }

@@ -8,7 +8,10 @@ namespace fdd {
 
 // ---------------------------------------------------------------------------------------
 // a2: in  uint8 [nsamps][nchans] (channel fastest)
-//     out float [nchans][rpitch], out[c][t] = in[t][c] for t < nsamps, 0 for nsamps <= t < nfft
+//     out float [nchans][rpitch], out[c][t] = in[t][c] - offset for t < nsamps, 0 for
+//     nsamps <= t < nfft.  offset (128 when nsamps == nfft, else 0; exact in fp32) takes the
+//     mean of unsigned-byte data out of the fp32 FFTs; a4 adds offset * nchans * nsamps back
+//     to bin 0 (k = 0 has phasor 1 for every trial DM), so the result is unchanged.
 // "transposed and unpacked ... in one kernel, thus requiring only a single pass",
 // "zero padded such that the number of samples becomes a power of two".
 // One CTA moves a 64 (time) x 64 (channel) tile through shared memory so that both the byte
@@ -19,7 +22,7 @@ constexpr int kUnpackTile = 64;
 template <int VEC>
 __global__ void __launch_bounds__(256)
 k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int nchans,
-                   long long nsamps, long long nfft, long long rpitch)
+                   long long nsamps, long long nfft, long long rpitch, float offset)
 {
     __shared__ float tile[kUnpackTile][kUnpackTile + 1];
     const int tid = threadIdx.x;
@@ -36,10 +39,10 @@ k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int 
             uchar4 v = make_uchar4(0, 0, 0, 0);
             if (t < nsamps && c0 + cq < nchans)
                 v = *reinterpret_cast<const uchar4*>(in + t * nchans + c0 + cq);
-            tile[cq + 0][tr] = (float)v.x;
-            tile[cq + 1][tr] = (float)v.y;
-            tile[cq + 2][tr] = (float)v.z;
-            tile[cq + 3][tr] = (float)v.w;
+            tile[cq + 0][tr] = (float)v.x - offset;
+            tile[cq + 1][tr] = (float)v.y - offset;
+            tile[cq + 2][tr] = (float)v.z - offset;
+            tile[cq + 3][tr] = (float)v.w - offset;
         }
     } else {
         const int trow = tid >> 6;          // 0..3
@@ -49,7 +52,7 @@ k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int 
             const int tr = trow + 4 * i;
             const long long t = t0 + tr;
             float v = 0.f;
-            if (t < nsamps && c0 + cc < nchans) v = (float)in[t * nchans + c0 + cc];
+            if (t < nsamps && c0 + cc < nchans) v = (float)in[t * nchans + c0 + cc] - offset;
             tile[cc][tr] = v;
         }
     }

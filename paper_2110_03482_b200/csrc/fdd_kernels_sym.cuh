@@ -155,7 +155,7 @@ k_rotate_sum_sym(const float2* __restrict__ X, long long xpitch,
                  const unsigned long long* __restrict__ centre64,
                  const unsigned long long* __restrict__ half64, int nchans, long long nbins,
                  int tile0, int ntiles, int ndm, float2* __restrict__ out, long long opitch,
-                 int row0, float scale, int real_edges)
+                 int row0, float scale, int real_edges, float dc_add)
 {
     // 1-D grid, DM tile fastest: CTAs resident together read the same X slab through L2.
     const int tile = tile0 + (int)(blockIdx.x % (unsigned)ntiles);
@@ -220,16 +220,17 @@ k_rotate_sum_sym(const float2* __restrict__ X, long long xpitch,
         if (!live[b]) continue;
         const long long k = kk[b];
         const bool edge = real_edges && (k == 0 || k == nbins - 1);
+        const float dc = k == 0 ? dc_add : 0.f;       // the mean a2 removed (already scaled)
 #pragma unroll
         for (int m = 0; m < kSymPairs; ++m) {
             const int jp = j0 + kSymPairs + m, jm = j0 + kSymPairs - 1 - m;
             if (jp < ndm)
                 out[(long long)(jp - row0) * opitch + k] =
-                    make_float2((U[b][m].x + V[b][m].y) * scale,
+                    make_float2((U[b][m].x + V[b][m].y) * scale + dc,
                                 edge ? 0.f : (V[b][m].x + U[b][m].y) * scale);
             if (jm < ndm)
                 out[(long long)(jm - row0) * opitch + k] =
-                    make_float2((U[b][m].x - V[b][m].y) * scale,
+                    make_float2((U[b][m].x - V[b][m].y) * scale + dc,
                                 edge ? 0.f : (V[b][m].x - U[b][m].y) * scale);
         }
     }
@@ -241,7 +242,7 @@ constexpr int kSymKT = 2;   // bins per thread
 // of kSymT (the plan's DM chunks are).
 inline int sym_launch(const SymTables& t, const float2* X, long long xpitch, int nchans,
                       long long nbins, int ndm, int j_begin, int rows, float2* dst, long long opitch,
-                      float scale, int real_edges, cudaStream_t s)
+                      float scale, int real_edges, float dc_add, cudaStream_t s)
 {
     if (j_begin % kSymT != 0 || !t.centre64) return -5;
     const int tile0 = j_begin / kSymT;
@@ -252,7 +253,7 @@ inline int sym_launch(const SymTables& t, const float2* X, long long xpitch, int
     if ((long long)ntl * nkb > 2147483647LL) return -5;
     k_rotate_sum_sym<kSymKT><<<(unsigned)(ntl * nkb), kSymThreads, 0, s>>>(
         X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ntl, row_end, dst, opitch, j_begin,
-        scale, real_edges);
+        scale, real_edges, dc_add);
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
 

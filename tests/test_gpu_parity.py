@@ -65,7 +65,8 @@ def test_unpack_and_r2c_against_fp64_rfft(F, nchans, nsamps):
         out = torch.empty((1, plan.nsamps), dtype=torch.float32, device="cuda")
         plan.execute(d_in, out, F.FDD_MODE_TIME)
         torch.cuda.synchronize()
-        ptr, pitch = plan.get_spectrum()
+        ptr, pitch, dc_removed = plan.get_spectrum()
+        assert dc_removed == (128.0 * nsamps if nsamps == plan.nfft else 0.0)
         assert plan.nfft == O.next_pow2(nsamps) and plan.nbins == plan.nfft // 2 + 1
         # view the plan's X in place through the CUDA array interface
         class _View:
@@ -74,6 +75,7 @@ def test_unpack_and_r2c_against_fp64_rfft(F, nchans, nsamps):
         xs = torch.as_tensor(_View(), device="cuda")
         X = xs.cpu().numpy()
         X = (X[..., 0] + 1j * X[..., 1])[:, :plan.nbins]
+        X[:, 0] += dc_removed                      # the mean a2 takes out of the fp32 FFT
         ref = np.fft.rfft(O.unpack(u8, plan.nfft), axis=-1)
         # fp32 FFT of u8 data: error relative to the rms of the non-DC bins
         rms = np.sqrt((np.abs(ref[:, 1:]) ** 2).mean())
