@@ -65,7 +65,9 @@ enum fdd_status {
 enum fdd_kernel {
     FDD_KERNEL_AUTO = 0,       /* symmetric kernel where the DM grid allows it, else generic     */
     FDD_KERNEL_GENERIC = 1,    /* any delay table: one exactly range-reduced phasor per element  */
-    FDD_KERNEL_SYMMETRIC = 2   /* DM tiles in arithmetic progression: paired +-m rows */
+    FDD_KERNEL_SYMMETRIC = 2,  /* DM tiles in arithmetic progression: paired +-m rows */
+    FDD_KERNEL_SYMMETRIC2 = 3  /* same, two adjacent 32-DM tiles per CTA sharing one phasor
+                                  recurrence; needs one DM step across each 64-DM tile pair      */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */
@@ -96,7 +98,9 @@ int fdd_plan_create_from_delays(fdd_plan **plan_out, int nchans, long long nsamp
 int fdd_plan_set_kdm(fdd_plan *plan, double k_dm);
 
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
- * for a delay table that is not in arithmetic progression within every DM tile. */
+ * for a delay table that is not in arithmetic progression within every 32-DM tile, or
+ * FDD_KERNEL_SYMMETRIC2 for one whose step changes inside a 64-DM tile pair.  AUTO takes the
+ * fastest kernel the table allows: SYMMETRIC2, else SYMMETRIC, else GENERIC. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 
 /* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy

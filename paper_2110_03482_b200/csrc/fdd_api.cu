@@ -15,6 +15,7 @@
 #include "fdd_kernels_generic.cuh"
 #include "fdd_kernels_pre.cuh"
 #include "fdd_kernels_sym.cuh"
+#include "fdd_kernels_sym2.cuh"
 
 namespace {
 
@@ -144,6 +145,19 @@ inline unsigned long long cycles_to_fixed64(long double cyc)
     return (unsigned long long)(s + 0.5L);
 }
 
+// AUTO: the fastest kernel the delay table allows.
+int resolve_kernel(const fdd_plan* p, int request)
+{
+    const bool sym2_ok = p->sym_ok && p->sym.pair_ok;
+    switch (request) {
+        case FDD_KERNEL_GENERIC: return FDD_KERNEL_GENERIC;
+        case FDD_KERNEL_SYMMETRIC: return p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC;
+        default:
+            return sym2_ok ? FDD_KERNEL_SYMMETRIC2
+                           : (p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC);
+    }
+}
+
 int upload_generic_table(fdd_plan* p)
 {
     std::vector<unsigned long long> tab((size_t)p->nchans * p->ndm_pad, 0ULL);
@@ -167,8 +181,7 @@ int build_tables(fdd_plan* p)
     rc = fdd::sym_build_tables(&p->sym, p->delays.data(), p->ndm, p->nchans, p->nfft, &p->sym_ok,
                                &p->scratch_bytes);
     if (rc != FDD_OK) return rc;
-    p->kernel = (p->kernel_request == FDD_KERNEL_GENERIC || !p->sym_ok) ? FDD_KERNEL_GENERIC
-                                                                        : FDD_KERNEL_SYMMETRIC;
+    p->kernel = resolve_kernel(p, p->kernel_request);
     return FDD_OK;
 }
 
@@ -357,7 +370,10 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
-    if (p->kernel == FDD_KERNEL_SYMMETRIC)
+    if (p->kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % (2 * fdd::kSymT) == 0)
+        return fdd::sym2_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
+                                dst, opitch, scale, real_edges, dc_add, s);
+    if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
@@ -524,12 +540,11 @@ int fdd_plan_set_kdm(fdd_plan* p, double k_dm)
 int fdd_plan_set_kernel(fdd_plan* p, int kernel)
 {
     if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
-    if (kernel != FDD_KERNEL_AUTO && kernel != FDD_KERNEL_GENERIC && kernel != FDD_KERNEL_SYMMETRIC)
-        return FDD_ERR_INVALID_ARG;
+    if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_SYMMETRIC2) return FDD_ERR_INVALID_ARG;
     if (kernel == FDD_KERNEL_SYMMETRIC && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
+    if (kernel == FDD_KERNEL_SYMMETRIC2 && !(p->sym_ok && p->sym.pair_ok)) return FDD_ERR_UNSUPPORTED;
     p->kernel_request = kernel;
-    p->kernel = (kernel == FDD_KERNEL_GENERIC || !p->sym_ok) ? FDD_KERNEL_GENERIC
-                                                             : FDD_KERNEL_SYMMETRIC;
+    p->kernel = resolve_kernel(p, kernel);
     return FDD_OK;
 }
 

@@ -48,7 +48,27 @@ struct SymTables {
     unsigned long long* half64 = nullptr;     // [ntiles][nchans] frac(h_c / nfft) * 2^64
     int ntiles = 0;
     size_t bytes = 0;
+    bool pair_ok = false;   // sub-tiles 2t and 2t+1 share the half step (fdd_kernels_sym2.cuh)
 };
+
+// Do sub-tiles 2t and 2t+1 form one arithmetic progression in every channel: same half step,
+// and centre(2t+1) = centre(2t) + 64 half steps?  (host, plan time; fdd_kernels_sym2.cuh)
+inline bool sym_pairs_share_step(const std::vector<unsigned long long>& centre64,
+                                 const std::vector<unsigned long long>& half64, int ntiles,
+                                 int nchans)
+{
+    // units of 2^-64 cycle per bin; bins < 2^31: 2^20 is < 1e-4 cycles of phase anywhere
+    auto near0 = [](unsigned long long d) { return d <= (1ULL << 20) || d >= ~0ULL - (1ULL << 20); };
+    for (int t = 0; t + 1 < ntiles; t += 2)
+        for (int c = 0; c < nchans; ++c) {
+            const unsigned long long ha = half64[(size_t)t * nchans + c];
+            const unsigned long long hb = half64[(size_t)(t + 1) * nchans + c];
+            const unsigned long long ca = centre64[(size_t)t * nchans + c];
+            const unsigned long long cb = centre64[(size_t)(t + 1) * nchans + c];
+            if (!near0(ha - hb) || !near0(cb - ca - (ha << 6))) return false;
+        }
+    return true;
+}
 
 inline void sym_free_tables(SymTables* t)
 {
@@ -57,6 +77,7 @@ inline void sym_free_tables(SymTables* t)
     t->centre64 = t->half64 = nullptr;
     t->ntiles = 0;
     t->bytes = 0;
+    t->pair_ok = false;
 }
 
 inline unsigned long long sym_fixed64(long double cyc)
@@ -109,6 +130,7 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
         return -3;
     }
     t->ntiles = ntiles;
+    t->pair_ok = sym_pairs_share_step(hc, hh, ntiles, nchans);
     t->bytes = 2 * bytes;
     if (scratch_bytes) *scratch_bytes += t->bytes;
     *ok = true;

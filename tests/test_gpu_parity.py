@@ -48,10 +48,17 @@ def _delays_for(w):
     return O.delay_table(w.nchans, w.f_lo, w.f_hi, w.tsamp, w.dm_list)
 
 
-KERNELS = ["generic", "auto"]
+KERNELS = ["generic", "symmetric", "auto"]
 
 
 def _set_kernel(F, plan, which):
+    """auto = the fastest kernel the delay table allows (SYMMETRIC2 on uniform DM grids)."""
+    if which == "symmetric":
+        try:
+            plan.set_kernel(F.FDD_KERNEL_SYMMETRIC)
+        except F.FddError:
+            pytest.skip("delay table is not an arithmetic progression per DM tile")
+        return
     plan.set_kernel(F.FDD_KERNEL_GENERIC if which == "generic" else F.FDD_KERNEL_AUTO)
 
 
@@ -116,6 +123,8 @@ RAGGED = [
     (33, 4096, 37, 1.25, -5.0),      # negative DMs, ndm ragged against every tile size
     (96, 6000, 70, 0.9, 3.3),        # padded 6000 -> 8192, two DM tiles + tail
     (2, 2, 2, 1.0, 0.0),             # smallest legal nsamps
+    (1100, 512, 40, 0.5, 0.0),       # more channels than one shared-memory table chunk (1024)
+    (40, 1024, 129, 0.25, 1.0),      # five 32-DM tiles: two tile pairs + an odd tail tile
 ]
 
 
@@ -152,6 +161,28 @@ def test_non_uniform_dm_list_and_kdm_override(F):
         assert np.abs(plan.get_delays() - d).max() <= 1e-9
         got = _run(F, plan, u8, "time")
     parity.assert_rows(got, ref, "time", "non-uniform DM list")
+
+
+def test_kernel_selection_follows_the_dm_grid(F):
+    """AUTO: SYMMETRIC2 on one uniform grid, SYMMETRIC when the step changes between 32-DM tiles
+    (a piecewise-uniform DM plan), GENERIC otherwise; each against the fp64 oracle."""
+    w = synth.small_workload(78, 40, 2048, 2)
+    u8 = synth.make_filterbank(w)
+    uniform = np.arange(96) * 0.75
+    piecewise = np.concatenate([np.arange(32) * 0.5, 16.0 + np.arange(32) * 1.0,
+                                48.0 + np.arange(20) * 2.0])
+    random = np.sort(np.random.default_rng(6).uniform(0, 80, size=70))
+    for dms, want in ((uniform, F.FDD_KERNEL_SYMMETRIC2), (piecewise, F.FDD_KERNEL_SYMMETRIC),
+                      (random, F.FDD_KERNEL_GENERIC)):
+        d = O.delay_table(40, w.f_lo, w.f_hi, w.tsamp, dms)
+        ref = O.fdd_fft(u8, d)
+        with F.Plan.create(40, 2048, w.tsamp, w.f_lo, w.f_hi, dms) as plan:
+            assert plan.get_info()[5] == want
+            if want != F.FDD_KERNEL_SYMMETRIC2:
+                with pytest.raises(F.FddError):
+                    plan.set_kernel(F.FDD_KERNEL_SYMMETRIC2)
+            got = _run(F, plan, u8, "time")
+        parity.assert_rows(got, ref, "time", f"kernel selection {want}")
 
 
 # ------------------------------------------------------------------ P3 on the GPU: exact integers
