@@ -24,6 +24,7 @@ namespace fdd {
 
 constexpr int kSym2Threads = 128;
 constexpr int kSym2Chunk = 1024;       // channels whose phase steps are staged in shared memory
+constexpr int kSym2Depth = 8;          // X prefetch queue depth (channels in flight per thread)
 
 struct Sym2Seed {
     float zrA, ziA, zrB, ziB;
@@ -31,29 +32,26 @@ struct Sym2Seed {
     float c2;
 };
 
-// Top 32 bits of (p64 * k mod 2^64) and the full product: the exact fractional cycle of k*P.
-__device__ __forceinline__ unsigned long long sym2_mul(uint2 p, unsigned int k)
-{
-    const unsigned long long w = (unsigned long long)p.x * k;           // lo * k
-    const unsigned int top = p.y * k + (unsigned int)(w >> 32);          // (hi * k + carry) mod 2^32
-    return ((unsigned long long)top << 32) | (unsigned int)w;
-}
 
 __device__ __forceinline__ float sym2_rad(unsigned int top)
 {
     return (float)(int)top * 1.4629180792671596e-09f;                    // 2 pi * 2^-32
 }
 
-// Seed of one (channel, bin): centre phases of sub-tiles A and B = A + 64 half steps, pair phasor
-// E_0 = (cos, sin) phi and c2 = 2 cos 2 phi.
-__device__ __forceinline__ Sym2Seed sym2_seed(float2 x, uint2 pa, uint2 ph, unsigned int k)
+// Seed of one (channel, bin) from the phase steps p = (centre A lo, hi, half step lo, hi), each a
+// 64-bit binary fraction of a cycle per bin: k * P mod 2^64 is the exact fractional cycle; its
+// top 32 bits feed the SFU.  Centre of sub-tile B = centre A + 64 half steps (a carry out of the
+// low words is 2^-32 cycle and dropped).  E_0 = (cos, sin) phi, c2 = 2 cos 2 phi.
+__device__ __forceinline__ Sym2Seed sym2_seed(float2 x, uint4 p, unsigned int k)
 {
-    const unsigned long long ta = sym2_mul(pa, k), th = sym2_mul(ph, k);
-    const unsigned long long tb = ta + (th << 6);
+    const unsigned int ta = p.y * k + __umulhi(p.x, k);
+    const unsigned long long wh = (unsigned long long)p.z * k;
+    const unsigned int th = p.w * k + (unsigned int)(wh >> 32);
+    const unsigned int tb = ta + __funnelshift_l((unsigned int)wh, th, 6);
     float sa, ca, sb, cb, b0, a0;
-    __sincosf(sym2_rad((unsigned int)(ta >> 32)), &sa, &ca);
-    __sincosf(sym2_rad((unsigned int)(tb >> 32)), &sb, &cb);
-    __sincosf(sym2_rad((unsigned int)(th >> 32)), &b0, &a0);
+    __sincosf(sym2_rad(ta), &sa, &ca);
+    __sincosf(sym2_rad(tb), &sb, &cb);
+    __sincosf(sym2_rad(th), &b0, &a0);
     Sym2Seed s;
     s.zrA = fmaf(x.x, ca, -x.y * sa);
     s.ziA = fmaf(x.x, sa, x.y * ca);
@@ -66,6 +64,56 @@ __device__ __forceinline__ Sym2Seed sym2_seed(float2 x, uint2 pa, uint2 ph, unsi
     return s;
 }
 
+// One channel: 64 accumulate + 15 recurrence FFMA2 with the seed `cur`.
+__device__ __forceinline__ void sym2_accumulate(const Sym2Seed& cur, float2 (&UA)[kSymPairs],
+                                                float2 (&VA)[kSymPairs], float2 (&UB)[kSymPairs],
+                                                float2 (&VB)[kSymPairs])
+{
+    const float2 zrA = make_float2(cur.zrA, cur.zrA), ziA = make_float2(cur.ziA, cur.ziA);
+    const float2 zrB = make_float2(cur.zrB, cur.zrB), ziB = make_float2(cur.ziB, cur.ziB);
+    const float2 c2 = make_float2(cur.c2, cur.c2);
+    // The recurrence runs one step ahead of the accumulation, so an accumulate FFMA2 never
+    // issues right behind the FFMA2 that produces its phasor (that would stall a full FFMA2
+    // latency fifteen times per channel).
+    float2 ep = make_float2(cur.e0.x, -cur.e0.y);     // E_{-1} = conj(E_0)
+    float2 e = cur.e0;                                // E_m
+    float2 en = __ffma2_rn(c2, e, make_float2(-ep.x, -ep.y));   // E_{m+1}
+#pragma unroll
+    for (int m = 0; m < kSymPairs; ++m) {
+        float2 enn = en;
+        if (m + 2 < kSymPairs) enn = __ffma2_rn(c2, en, make_float2(-e.x, -e.y));   // E_{m+2}
+        UA[m] = __ffma2_rn(zrA, e, UA[m]);
+        VA[m] = __ffma2_rn(ziA, e, VA[m]);
+        UB[m] = __ffma2_rn(zrB, e, UB[m]);
+        VB[m] = __ffma2_rn(ziB, e, VB[m]);
+        e = en;
+        en = enn;
+    }
+}
+
+__device__ __forceinline__ void sym2_cp_async8(unsigned int saddr, const float2* g)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void sym2_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void sym2_cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ float2 sym2_lds_x(unsigned int addr)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ uint4 sym2_lds(unsigned int addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+
 __global__ void __launch_bounds__(kSym2Threads, 3)
 k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   const unsigned long long* __restrict__ centre64,
@@ -73,10 +121,11 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   int tile0, int npairs, int ntiles_total, int ndm, float2* __restrict__ out,
                   long long opitch, int row0, float scale, int real_edges, float dc_add)
 {
-    // Phase steps of the channels in flight.  They are the same for every thread, so they are
-    // staged once per CTA: a global load of them inside the channel loop would share a
-    // scoreboard with the X prefetch and expose its full L2/HBM latency every iteration.
-    __shared__ uint2 s_pa[kSym2Chunk + 1], s_ph[kSym2Chunk + 1];
+    // Phase steps of the channels in flight, (centre A, half step) per channel.  They are the
+    // same for every thread, so they are staged once per CTA: a global load of them inside the
+    // channel loop would share a scoreboard with the X prefetch and expose its latency.
+    __shared__ uint4 s_p[kSym2Chunk + 2];
+    __shared__ float2 s_x[kSym2Depth][kSym2Threads];
 
     // 1-D grid, DM tile-pair fastest: CTAs resident together read the same X slab through L2.
     const int pr = (int)(blockIdx.x % (unsigned)npairs);
@@ -94,48 +143,50 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
 
     const uint2* ga = reinterpret_cast<const uint2*>(centre64 + (size_t)tA * nchans);
     const uint2* gh = reinterpret_cast<const uint2*>(half64 + (size_t)tA * nchans);
-    const unsigned int ku = (unsigned int)k;
-    const float2* xq = X + k + 2 * xpitch;            // channel c + 2 of the current iteration
+    unsigned int ku = (unsigned int)k;
+    asm volatile("" : "+r"(ku));                      // keep k in a register (no re-derivation)
+    const unsigned int sbase = (unsigned int)__cvta_generic_to_shared(s_p);
+    const unsigned int xbase = (unsigned int)__cvta_generic_to_shared(&s_x[0][threadIdx.x]);
+
+    // X prefetch queue: every thread streams ITS OWN bin of the next kSym2Depth channels into its
+    // own shared-memory slots with cp.async (no thread reads another's slot, so no barrier):
+    // registers hold one X value, the queue covers L2 / HBM latency of kSym2Depth iterations.
+    const float2* xq = X + k + xpitch;                // next channel to request (1, 2, ...)
+    int to_request = nchans - 1;
+#pragma unroll
+    for (int d = 1; d < kSym2Depth; ++d) {
+        if (to_request > 0) sym2_cp_async8(xbase + d * (kSym2Threads * 8), xq);
+        sym2_cp_commit();
+        xq += xpitch;
+        --to_request;
+    }
 
     Sym2Seed cur;
-    float2 x1;
+    int slot = 1;                                     // queue slot of channel c + 1
     for (int c0 = 0; c0 < nchans; c0 += kSym2Chunk) {
         const int n = nchans - c0 < kSym2Chunk ? nchans - c0 : kSym2Chunk;
         __syncthreads();
         for (int i = threadIdx.x; i <= n; i += kSym2Threads) {
             const int cc = c0 + i < nchans ? c0 + i : nchans - 1;
-            s_pa[i] = __ldg(ga + cc);
-            s_ph[i] = __ldg(gh + cc);
+            const uint2 a = __ldg(ga + cc), h = __ldg(gh + cc);
+            s_p[i] = make_uint4(a.x, a.y, h.x, h.y);
         }
         __syncthreads();
-        if (c0 == 0) {
-            cur = sym2_seed(X[k], s_pa[0], s_ph[0], ku);
-            x1 = X[(nchans > 1 ? xpitch : 0) + k];
-        }
+        if (c0 == 0) cur = sym2_seed(X[k], s_p[0], ku);
+        unsigned int sp = sbase + 16;                 // table entry of channel c + 1
         for (int i = 0; i < n; ++i) {
-            float2 x2 = x1;
-            if (c0 + i + 2 < nchans) x2 = *xq;        // two channels ahead
+            // channel c + kSym2Depth goes into the slot channel c left in the last iteration
+            const int wslot = slot == 0 ? kSym2Depth - 1 : slot - 1;
+            if (to_request > 0) sym2_cp_async8(xbase + wslot * (kSym2Threads * 8), xq);
+            sym2_cp_commit();
             xq += xpitch;
-
-            const float2 zrA = make_float2(cur.zrA, cur.zrA), ziA = make_float2(cur.ziA, cur.ziA);
-            const float2 zrB = make_float2(cur.zrB, cur.zrB), ziB = make_float2(cur.ziB, cur.ziB);
-            const float2 c2 = make_float2(cur.c2, cur.c2);
-            float2 e = cur.e0;
-            float2 ep = make_float2(e.x, -e.y);       // E_{-1} = conj(E_0)
-#pragma unroll
-            for (int m = 0; m < kSymPairs; ++m) {
-                UA[m] = __ffma2_rn(zrA, e, UA[m]);
-                VA[m] = __ffma2_rn(ziA, e, VA[m]);
-                UB[m] = __ffma2_rn(zrB, e, UB[m]);
-                VB[m] = __ffma2_rn(ziB, e, VB[m]);
-                if (m + 1 < kSymPairs) {
-                    const float2 en = __ffma2_rn(c2, e, make_float2(-ep.x, -ep.y));
-                    ep = e;
-                    e = en;
-                }
-            }
-            cur = sym2_seed(x1, s_pa[i + 1], s_ph[i + 1], ku);
-            x1 = x2;
+            --to_request;
+            sym2_accumulate(cur, UA, VA, UB, VB);     // channel c
+            sym2_cp_wait<kSym2Depth - 1>();           // channel c + 1 has landed
+            const float2 x1 = sym2_lds_x(xbase + slot * (kSym2Threads * 8));
+            cur = sym2_seed(x1, sym2_lds(sp), ku);    // seed of channel c + 1
+            sp += 16;
+            slot = slot + 1 == kSym2Depth ? 0 : slot + 1;
         }
     }
     if (!live) return;
