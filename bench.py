@@ -321,14 +321,13 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     sum_ms = stage_ms["rotate_sum"] / args.steps
     achieved = FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")   # from the committed ncu summaries
     if os.path.exists(tpath):
-        try:
-            tj = json.load(open(tpath))
-            key = f"{w.name}/{w.ndm}/kernel{kernel}"
-            traffic = tj.get(key)
-        except Exception:
-            traffic = None
+        key = f"{w.name}/{w.ndm}/kernel{kernel}"
+        for ln in open(tpath):
+            f = ln.strip().split(",")
+            if len(f) >= 2 and f[0] == key:
+                traffic = float(f[1])
     # FMA lanes the kernel actually executes per element (accumulate + phasor recurrence):
     # sym2 79 FFMA2 per 64 DMs, sym 47 FFMA2 per 32 DMs, generic 4 FFMA per element
     kname, fma_lanes = {F.FDD_KERNEL_SYMMETRIC2: ("k_rotate_sum_sym2", 79 * 2 / 64.0),
