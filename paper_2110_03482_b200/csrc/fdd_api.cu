@@ -22,8 +22,8 @@ namespace {
 constexpr double kDefaultKdm = 4.148808e3;            // MHz^2 pc^-1 cm^3 s (reading S5)
 constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
 constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
-constexpr int kC2RBatch = 256;                        // rows per cuFFT C2R call (bounds workspace)
-constexpr int kHostChunkRows = 2 * kC2RBatch;         // fdd_execute_host: DM rows per pipelined chunk
+constexpr int kC2RBatch = 128;                        // rows per cuFFT C2R call (bounds workspace)
+constexpr int kHostChunkRows = 3 * kC2RBatch;         // fdd_execute_host: DM rows per pipelined chunk
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
@@ -230,7 +230,8 @@ int ensure_time_resources(fdd_plan* p)
         if (fit < rows) rows = fit;
     }
     if (rows >= p->ndm) rows = p->ndm;
-    else rows = rows / kC2RBatch * kC2RBatch;
+    else rows = rows >= 3 * kC2RBatch ? rows / (3 * kC2RBatch) * (3 * kC2RBatch)   // whole 96-DM groups
+                                      : rows / kC2RBatch * kC2RBatch;
     if (rows < 1) return FDD_ERR_ALLOC;
     p->y_rows = (int)rows;
     p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
@@ -370,9 +371,17 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
-    if (p->kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % (2 * fdd::kSymT) == 0)
-        return fdd::sym2_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
-                                dst, opitch, scale, real_edges, dc_add, s);
+    if (p->kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
+        // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of
+        // one group per (channel, warp): 315 cycles for NS = 3, 232 for NS = 2
+        const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
+        const long long cost3 = (long long)((ntl + 2) / 3) * 315, cost2 = (long long)((ntl + 1) / 2) * 232;
+        if (cost3 <= cost2)
+            return fdd::sym2_launch<3, 2>(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+                                          rows, dst, opitch, scale, real_edges, dc_add, s);
+        return fdd::sym2_launch<2, 3>(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+                                      rows, dst, opitch, scale, real_edges, dc_add, s);
+    }
     if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);

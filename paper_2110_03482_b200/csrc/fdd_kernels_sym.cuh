@@ -48,18 +48,19 @@ struct SymTables {
     unsigned long long* half64 = nullptr;     // [ntiles][nchans] frac(h_c / nfft) * 2^64
     int ntiles = 0;
     size_t bytes = 0;
-    bool pair_ok = false;   // sub-tiles 2t and 2t+1 share the half step (fdd_kernels_sym2.cuh)
+    bool pair_ok = false;   // adjacent sub-tiles continue one progression (fdd_kernels_sym2.cuh)
 };
 
-// Do sub-tiles 2t and 2t+1 form one arithmetic progression in every channel: same half step,
-// and centre(2t+1) = centre(2t) + 64 half steps?  (host, plan time; fdd_kernels_sym2.cuh)
+// Do all adjacent sub-tiles t, t+1 continue one arithmetic progression in every channel: same half
+// step, and centre(t+1) = centre(t) + 64 half steps?  (host, plan time; fdd_kernels_sym2.cuh groups
+// two or three adjacent sub-tiles from any chunk start)
 inline bool sym_pairs_share_step(const std::vector<unsigned long long>& centre64,
                                  const std::vector<unsigned long long>& half64, int ntiles,
                                  int nchans)
 {
     // units of 2^-64 cycle per bin; bins < 2^31: 2^20 is < 1e-4 cycles of phase anywhere
     auto near0 = [](unsigned long long d) { return d <= (1ULL << 20) || d >= ~0ULL - (1ULL << 20); };
-    for (int t = 0; t + 1 < ntiles; t += 2)
+    for (int t = 0; t + 1 < ntiles; ++t)
         for (int c = 0; c < nchans; ++c) {
             const unsigned long long ha = half64[(size_t)t * nchans + c];
             const unsigned long long hb = half64[(size_t)(t + 1) * nchans + c];
@@ -103,8 +104,10 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
         const int r = ndm - j0 < kSymT ? ndm - j0 : kSymT;
         for (int c = 0; c < nchans; ++c) {
             const long double d0 = delays[(size_t)j0 * nchans + c];
+            // a one-row tail tile continues the step of the row before it (any step fits one row)
             const long double step =
-                r >= 2 ? ((long double)delays[(size_t)(j0 + r - 1) * nchans + c] - d0) / (r - 1) : 0.0L;
+                r >= 2 ? ((long double)delays[(size_t)(j0 + r - 1) * nchans + c] - d0) / (r - 1)
+                       : (j0 > 0 ? d0 - (long double)delays[(size_t)(j0 - 1) * nchans + c] : 0.0L);
             for (int i = 1; i < r; ++i) {
                 const long double want = d0 + step * i;
                 const long double got = delays[(size_t)(j0 + i) * nchans + c];
