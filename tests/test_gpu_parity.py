@@ -254,8 +254,9 @@ def _sampled_rows(ndm, n, seed):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("name,nrows", [("config2", 16), ("config3", 8)])
+@pytest.mark.parametrize("name,nrows", [("config2", 16), ("config3", 8), ("config4", 8)])
 def test_full_size_time_configs(F, oracle_c, name, nrows):
+    """config4 = the 4096-DM sweep point bench.py times (same plan, same kernel choice)."""
     import torch
     w = synth.workload(name)
     u8 = synth.make_filterbank(w)
