@@ -377,9 +377,9 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
         const long long cost3 = (long long)((ntl + 2) / 3) * 315, cost2 = (long long)((ntl + 1) / 2) * 232;
         if (cost3 <= cost2)
-            return fdd::sym2_launch<3, 2>(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+            return fdd::sym2_launch<3, 2>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
                                           rows, dst, opitch, scale, real_edges, dc_add, s);
-        return fdd::sym2_launch<2, 3>(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+        return fdd::sym2_launch<2, 3>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
                                       rows, dst, opitch, scale, real_edges, dc_add, s);
     }
     if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)

@@ -60,18 +60,49 @@ struct Sym2Seed {
     float c2;
 };
 
-// Seed of one (channel, bin) from the phase steps p = (centre A lo, hi, half step lo, hi), each a
-// 64-bit binary fraction of a cycle per bin: k * P mod 2^64 is the exact fractional cycle; its
-// top 32 bits feed the SFU.  Centre of sub-tile s = centre A + 64 s half steps (a carry out of
-// the low words is 2^-32 cycle and dropped).  E_0 = (cos, sin) phi, c2 = 2 cos 2 phi from the
-// smaller of |cos|, |sin| (2 - 4 sin^2 = 4 cos^2 - 2).
-template <int NS>
-__device__ __forceinline__ Sym2Seed<NS> sym2_seed(float2 x, uint4 p, unsigned int k)
+// The three 32-bit phases (fractions of a cycle * 2^32) of one (channel, bin): centre of sub-tile A,
+// half step, and 64 half steps (the distance between sub-tile centres), from the staged table
+// entry at shared address sp.  Two table formats:
+//  kFp64 (nfft <= 2^21): entry = (P_A, P_h, frac(64 P_h)) * 2^32 as doubles, P in [-1/2, 1/2)
+//    cycles per bin.  The low word of fma(k, P 2^32, 1.5 * 2^52) is round(k P 2^32) mod 2^32
+//    (|k P 2^32| < 2^51 for k <= 2^20): ONE instruction on the otherwise idle FP64 pipe per phase.
+//    The integer form costs an IMAD.HI/IMAD.WIDE + IMAD per phase in the FMA pipe the accumulation
+//    needs (measured: 195 -> 186 ms at config 4 / 4096 DMs).
+//  !kFp64 (any nfft): entry = (P_A lo, hi, P_h lo, hi), 64-bit binary fractions; k * P mod 2^64
+//    by integer multiplies, a carry out of the low words into 64 P_h (2^-32 cycle) dropped.
+struct Sym2Phases {
+    unsigned int ta, th, step;
+};
+
+template <bool kFp64>
+__device__ __forceinline__ Sym2Phases sym2_phases(unsigned int sp, unsigned int ku, double kd)
 {
-    const unsigned int ta = p.y * k + __umulhi(p.x, k);
-    const unsigned long long wh = (unsigned long long)p.z * k;
-    const unsigned int th = p.w * k + (unsigned int)(wh >> 32);
-    const unsigned int step = __funnelshift_l((unsigned int)wh, th, 6);   // 64 half steps
+    Sym2Phases ph;
+    if (kFp64) {
+        const double magic = 6755399441055744.0;                         // 1.5 * 2^52
+        double pa, p_h, p64h;
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(pa), "=d"(p_h) : "r"(sp));
+        asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(p64h) : "r"(sp));
+        ph.ta = (unsigned int)__double2loint(fma(kd, pa, magic));
+        ph.th = (unsigned int)__double2loint(fma(kd, p_h, magic));
+        ph.step = (unsigned int)__double2loint(fma(kd, p64h, magic));
+    } else {
+        const uint4 p = sym2_lds(sp);
+        ph.ta = p.y * ku + __umulhi(p.x, ku);
+        const unsigned long long wh = (unsigned long long)p.z * ku;
+        ph.th = p.w * ku + (unsigned int)(wh >> 32);
+        ph.step = __funnelshift_l((unsigned int)wh, ph.th, 6);
+    }
+    return ph;
+}
+
+// Seed of one (channel, bin): Z_s = X e^{i theta_s} for the NS sub-tile centres theta_s = theta_A +
+// s * (64 half steps), E_0 = (cos, sin) phi, c2 = 2 cos 2 phi from the smaller of |cos|, |sin|
+// (2 - 4 sin^2 = 4 cos^2 - 2).  The top 32 bits of each exact fractional cycle feed the SFU.
+template <int NS>
+__device__ __forceinline__ Sym2Seed<NS> sym2_seed(float2 x, Sym2Phases ph)
+{
+    const unsigned int ta = ph.ta, th = ph.th, step = ph.step;
     Sym2Seed<NS> s;
     unsigned int t = ta;
 #pragma unroll
@@ -118,7 +149,7 @@ __device__ __forceinline__ void sym2_accumulate(const Sym2Seed<NS>& cur, float2 
     }
 }
 
-template <int NS, int kMinCtas>
+template <int NS, int kMinCtas, bool kFp64>
 __global__ void __launch_bounds__(kSym2Threads, kMinCtas)
 k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   const unsigned long long* __restrict__ centre64,
@@ -129,7 +160,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
     // Phase steps of the channels in flight, (centre A, half step) per channel.  They are the
     // same for every thread, so they are staged once per CTA: a global load of them inside the
     // channel loop would share a scoreboard with the X prefetch and expose its latency.
-    __shared__ uint4 s_p[kSym2Chunk + 2];
+    __shared__ double4 s_p[kSym2Chunk + 2];         // 32 B per channel, format: sym2_phases
     __shared__ float2 s_x[kSym2Depth][kSym2Threads];
 
     // 1-D grid, DM tile-group fastest: CTAs resident together read the same X slab through L2.
@@ -148,6 +179,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
 
     const uint2* ga = reinterpret_cast<const uint2*>(centre64 + (size_t)tA * nchans);
     const uint2* gh = reinterpret_cast<const uint2*>(half64 + (size_t)tA * nchans);
+    const double kd = (double)k;
     unsigned int ku = (unsigned int)k;
     asm volatile("" : "+r"(ku));                      // keep k in a register (no re-derivation)
     const unsigned int sbase = (unsigned int)__cvta_generic_to_shared(s_p);
@@ -174,11 +206,20 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
         for (int i = threadIdx.x; i <= n; i += kSym2Threads) {
             const int cc = c0 + i < nchans ? c0 + i : nchans - 1;
             const uint2 a = __ldg(ga + cc), h = __ldg(gh + cc);
-            s_p[i] = make_uint4(a.x, a.y, h.x, h.y);
+            if (kFp64) {
+                const unsigned long long ua = ((unsigned long long)a.y << 32) | a.x;
+                const unsigned long long uh = ((unsigned long long)h.y << 32) | h.x;
+                // signed 64-bit fractions of a cycle (wrap = reduction to [-1/2, 1/2)) times 2^-32
+                s_p[i] = make_double4((double)(long long)ua * 2.3283064365386963e-10,
+                                      (double)(long long)uh * 2.3283064365386963e-10,
+                                      (double)(long long)(uh << 6) * 2.3283064365386963e-10, 0.0);
+            } else {
+                *reinterpret_cast<uint4*>(&s_p[i]) = make_uint4(a.x, a.y, h.x, h.y);
+            }
         }
         __syncthreads();
-        if (c0 == 0) cur = sym2_seed<NS>(X[k], s_p[0], ku);
-        unsigned int sp = sbase + 16;                 // table entry of channel c + 1
+        if (c0 == 0) cur = sym2_seed<NS>(X[k], sym2_phases<kFp64>(sbase, ku, kd));
+        unsigned int sp = sbase + 32;                 // table entry of channel c + 1
         for (int i = 0; i < n; ++i) {
             const int wslot = slot == 0 ? kSym2Depth - 1 : slot - 1;
             if (to_request > 0) sym2_cp_async8(xbase + wslot * (kSym2Threads * 8), xq);
@@ -188,8 +229,8 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
             sym2_accumulate<NS>(cur, U, V);           // channel c
             sym2_cp_wait<kSym2Depth - 1>();           // channel c + 1 has landed
             const float2 x1 = sym2_lds_x(xbase + slot * (kSym2Threads * 8));
-            cur = sym2_seed<NS>(x1, sym2_lds(sp), ku);    // seed of channel c + 1
-            sp += 16;
+            cur = sym2_seed<NS>(x1, sym2_phases<kFp64>(sp, ku, kd));   // seed of channel c + 1
+            sp += 32;
             slot = slot + 1 == kSym2Depth ? 0 : slot + 1;
         }
     }
@@ -218,7 +259,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
 // Rows [j_begin, j_begin + rows) -> dst[(j - j_begin) * opitch + k]; j_begin a multiple of kSymT.
 // The sub-tiles of the chunk are grouped NS at a time from its first one.
 template <int NS, int kMinCtas>
-inline int sym2_launch(const SymTables& t, const float2* X, long long xpitch, int nchans,
+inline int sym2_launch(long long nfft, const SymTables& t, const float2* X, long long xpitch, int nchans,
                        long long nbins, int ndm, int j_begin, int rows, float2* dst,
                        long long opitch, float scale, int real_edges, float dc_add, cudaStream_t s)
 {
@@ -230,9 +271,14 @@ inline int sym2_launch(const SymTables& t, const float2* X, long long xpitch, in
     const int ntiles_total = tile0 + ntl;             // sub-tiles past this chunk are not touched
     const long long nkb = (nbins + kSym2Threads - 1) / kSym2Threads;
     if ((long long)ngroups * nkb > 2147483647LL) return -5;
-    k_rotate_sum_sym2<NS, kMinCtas><<<(unsigned)(ngroups * nkb), kSym2Threads, 0, s>>>(
-        X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst,
-        opitch, j_begin, scale, real_edges, dc_add);
+    if (nfft <= (1LL << 21))
+        k_rotate_sum_sym2<NS, kMinCtas, true><<<(unsigned)(ngroups * nkb), kSym2Threads, 0, s>>>(
+            X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst,
+            opitch, j_begin, scale, real_edges, dc_add);
+    else
+        k_rotate_sum_sym2<NS, kMinCtas, false><<<(unsigned)(ngroups * nkb), kSym2Threads, 0, s>>>(
+            X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst,
+            opitch, j_begin, scale, real_edges, dc_add);
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
 

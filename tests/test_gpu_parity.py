@@ -124,7 +124,7 @@ RAGGED = [
     (96, 6000, 70, 0.9, 3.3),        # padded 6000 -> 8192, two DM tiles + tail
     (2, 2, 2, 1.0, 0.0),             # smallest legal nsamps
     (1100, 512, 40, 0.5, 0.0),       # more channels than one shared-memory table chunk (1024)
-    (40, 1024, 129, 0.25, 1.0),      # five 32-DM tiles: two tile pairs + an odd tail tile
+    (40, 1024, 129, 0.25, 1.0),      # five 32-DM tiles: a 96-DM group + a one-row tail tile
 ]
 
 
@@ -145,6 +145,20 @@ def test_ragged_shapes(F, nchans, nsamps, ndm, step, dm0, mode, kernel):
     else:
         scale = np.abs(ref).max()
         assert np.abs(got - ref).max() <= 1e-5 * scale
+
+
+@pytest.mark.parametrize("kernel", ["symmetric", "auto"])
+def test_long_series_use_the_integer_phase_variant(F, oracle_c, kernel):
+    """nfft = 2^22 > 2^21: k_rotate_sum_sym2 switches from FP64-pipe to integer phase products."""
+    w = synth.small_workload(321, 6, 1 << 22, 70, dm_step=0.5, dm0=0.0)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = [0, 1, 15, 16, 31, 32, 63, 64, 69]
+    ref = O.fdd_rows(u8, d, rows, mode="time")
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        got = _run(F, plan, u8, "time")[rows]
+    parity.assert_rows(got, ref, "time", f"nfft 2^22/{kernel}")
 
 
 def test_non_uniform_dm_list_and_kdm_override(F):
