@@ -63,29 +63,34 @@ struct Sym2Seed {
 // The three 32-bit phases (fractions of a cycle * 2^32) of one (channel, bin): centre of sub-tile A,
 // half step, and 64 half steps (the distance between sub-tile centres), from the staged table
 // entry at shared address sp.  Two table formats:
-//  kFp64 (nfft <= 2^21): entry = (P_A, P_h, frac(64 P_h)) * 2^32 as doubles, P in [-1/2, 1/2)
-//    cycles per bin.  The low word of fma(k, P 2^32, 1.5 * 2^52) is round(k P 2^32) mod 2^32
-//    (|k P 2^32| < 2^51 for k <= 2^20): ONE instruction on the otherwise idle FP64 pipe per phase.
-//    The integer form costs an IMAD.HI/IMAD.WIDE + IMAD per phase in the FMA pipe the accumulation
-//    needs (measured: 195 -> 186 ms at config 4 / 4096 DMs).
+//  kFp64 (nfft <= 2^23): entry = (P_A, P_h, frac(64 P_h)) * 2^(32-pshift) as doubles, P in
+//    [-1/2, 1/2) cycles per bin, pshift = max(0, log2 nfft - 21).  The low word of
+//    fma(k, P 2^(32-pshift), 1.5 * 2^52) is round(k P 2^(32-pshift)) mod 2^32 (the product stays
+//    below 2^51 for k <= nfft/2); shifted left by pshift it is the phase to 2^-(32-pshift) cycle:
+//    ONE instruction on the otherwise idle FP64 pipe per phase.  The integer form costs an
+//    IMAD.HI/IMAD.WIDE + IMAD per phase in the FMA pipe the accumulation needs (measured:
+//    195 -> 186 ms at config 4 / 4096 DMs).
 //  !kFp64 (any nfft): entry = (P_A lo, hi, P_h lo, hi), 64-bit binary fractions; k * P mod 2^64
 //    by integer multiplies, a carry out of the low words into 64 P_h (2^-32 cycle) dropped.
 struct Sym2Phases {
     unsigned int ta, th, step;
 };
 
-template <bool kFp64>
-__device__ __forceinline__ Sym2Phases sym2_phases(unsigned int sp, unsigned int ku, double kd)
+// kMode 0: FP64-pipe phases, pshift = 0; 1: FP64-pipe phases, pshift > 0; 2: integer phases.
+template <int kMode>
+__device__ __forceinline__ Sym2Phases sym2_phases(unsigned int sp, unsigned int ku, double kd,
+                                                  int pshift)
 {
     Sym2Phases ph;
-    if (kFp64) {
+    if (kMode < 2) {
         const double magic = 6755399441055744.0;                         // 1.5 * 2^52
         double pa, p_h, p64h;
         asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(pa), "=d"(p_h) : "r"(sp));
         asm volatile("ld.shared.f64 %0, [%1+16];" : "=d"(p64h) : "r"(sp));
-        ph.ta = (unsigned int)__double2loint(fma(kd, pa, magic));
-        ph.th = (unsigned int)__double2loint(fma(kd, p_h, magic));
-        ph.step = (unsigned int)__double2loint(fma(kd, p64h, magic));
+        const int sh = kMode == 0 ? 0 : pshift;
+        ph.ta = (unsigned int)__double2loint(fma(kd, pa, magic)) << sh;
+        ph.th = (unsigned int)__double2loint(fma(kd, p_h, magic)) << sh;
+        ph.step = (unsigned int)__double2loint(fma(kd, p64h, magic)) << sh;
     } else {
         const uint4 p = sym2_lds(sp);
         ph.ta = p.y * ku + __umulhi(p.x, ku);
@@ -165,13 +170,14 @@ __device__ __forceinline__ void sym2_accumulate(const Sym2Seed<NS>& cur, float2 
     }
 }
 
-template <int NS, int kMinCtas, bool kFp64>
+template <int NS, int kMinCtas, int kMode>
 __global__ void __launch_bounds__(kSym2Threads, kMinCtas)
 k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   const unsigned long long* __restrict__ centre64,
                   const unsigned long long* __restrict__ half64, int nchans, long long nbins,
                   int tile0, int ngroups, int ntiles_total, int ndm, float2* __restrict__ out,
-                  long long opitch, int row0, float scale, int real_edges, float dc_add)
+                  long long opitch, int row0, float scale, int real_edges, float dc_add,
+                  int pshift)
 {
     // Phase steps of the channels in flight, (centre A, half step) per channel.  They are the
     // same for every thread, so they are staged once per CTA: a global load of them inside the
@@ -222,19 +228,20 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
         for (int i = threadIdx.x; i <= n; i += kSym2Threads) {
             const int cc = c0 + i < nchans ? c0 + i : nchans - 1;
             const uint2 a = __ldg(ga + cc), h = __ldg(gh + cc);
-            if (kFp64) {
+            if (kMode < 2) {
                 const unsigned long long ua = ((unsigned long long)a.y << 32) | a.x;
                 const unsigned long long uh = ((unsigned long long)h.y << 32) | h.x;
-                // signed 64-bit fractions of a cycle (wrap = reduction to [-1/2, 1/2)) times 2^-32
-                s_p[i] = make_double4((double)(long long)ua * 2.3283064365386963e-10,
-                                      (double)(long long)uh * 2.3283064365386963e-10,
-                                      (double)(long long)(uh << 6) * 2.3283064365386963e-10, 0.0);
+                // signed 64-bit fractions of a cycle (wrap = reduction to [-1/2, 1/2)) times
+                // 2^-(32+pshift)
+                const double sc = __hiloint2double((1023 - 32 - pshift) << 20, 0);
+                s_p[i] = make_double4((double)(long long)ua * sc, (double)(long long)uh * sc,
+                                      (double)(long long)(uh << 6) * sc, 0.0);
             } else {
                 *reinterpret_cast<uint4*>(&s_p[i]) = make_uint4(a.x, a.y, h.x, h.y);
             }
         }
         __syncthreads();
-        if (c0 == 0) cur = sym2_seed<NS>(X[k], sym2_phases<kFp64>(sbase, ku, kd));
+        if (c0 == 0) cur = sym2_seed<NS>(X[k], sym2_phases<kMode>(sbase, ku, kd, pshift));
         unsigned int sp = sbase + 32;                 // table entry of channel c + 1
         for (int i = 0; i < n; ++i) {
             const int wslot = slot == 0 ? kSym2Depth - 1 : slot - 1;
@@ -245,7 +252,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
             sym2_accumulate<NS>(cur, U, V);           // channel c
             sym2_cp_wait<kSym2Depth - 1>();           // channel c + 1 has landed
             const float2 x1 = sym2_lds_x(xbase + slot * (kSym2Threads * 8));
-            cur = sym2_seed<NS>(x1, sym2_phases<kFp64>(sp, ku, kd));   // seed of channel c + 1
+            cur = sym2_seed<NS>(x1, sym2_phases<kMode>(sp, ku, kd, pshift));   // seed of channel c + 1
             sp += 32;
             slot = slot + 1 == kSym2Depth ? 0 : slot + 1;
         }
@@ -287,14 +294,17 @@ inline int sym2_launch(long long nfft, const SymTables& t, const float2* X, long
     const int ntiles_total = tile0 + ntl;             // sub-tiles past this chunk are not touched
     const long long nkb = (nbins + kSym2Threads - 1) / kSym2Threads;
     if ((long long)ngroups * nkb > 2147483647LL) return -5;
-    if (nfft <= (1LL << 21))
-        k_rotate_sum_sym2<NS, kMinCtas, true><<<(unsigned)(ngroups * nkb), kSym2Threads, 0, s>>>(
-            X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst,
-            opitch, j_begin, scale, real_edges, dc_add);
-    else
-        k_rotate_sum_sym2<NS, kMinCtas, false><<<(unsigned)(ngroups * nkb), kSym2Threads, 0, s>>>(
-            X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst,
-            opitch, j_begin, scale, real_edges, dc_add);
+    int pshift = 0;                                   // FP64-pipe phases: see sym2_phases
+    while ((nfft >> pshift) > (1LL << 21)) ++pshift;
+    const unsigned grid = (unsigned)(ngroups * nkb);
+#define FDD_SYM2_LAUNCH(MODE)                                                                      \
+    k_rotate_sum_sym2<NS, kMinCtas, MODE><<<grid, kSym2Threads, 0, s>>>(                           \
+        X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst, \
+        opitch, j_begin, scale, real_edges, dc_add, pshift)
+    if (pshift == 0) FDD_SYM2_LAUNCH(0);
+    else if (pshift <= 2) FDD_SYM2_LAUNCH(1);         // nfft <= 2^23; longer: integer phases
+    else FDD_SYM2_LAUNCH(2);
+#undef FDD_SYM2_LAUNCH
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
 

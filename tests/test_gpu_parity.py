@@ -147,10 +147,11 @@ def test_ragged_shapes(F, nchans, nsamps, ndm, step, dm0, mode, kernel):
         assert np.abs(got - ref).max() <= 1e-5 * scale
 
 
-@pytest.mark.parametrize("kernel", ["symmetric", "auto"])
-def test_long_series_use_the_integer_phase_variant(F, oracle_c, kernel):
-    """nfft = 2^22 > 2^21: k_rotate_sum_sym2 switches from FP64-pipe to integer phase products."""
-    w = synth.small_workload(321, 6, 1 << 22, 70, dm_step=0.5, dm0=0.0)
+@pytest.mark.parametrize("log2n,kernel", [(22, "symmetric"), (22, "auto"), (24, "auto")])
+def test_long_series_phase_variants(F, oracle_c, log2n, kernel):
+    """k_rotate_sum_sym2 forms its phases on the FP64 pipe with a reduced scale for
+    2^21 < nfft <= 2^23 and by integer multiplies beyond; k_rotate_sum_sym always by integers."""
+    w = synth.small_workload(321, 4, 1 << log2n, 70, dm_step=0.5, dm0=0.0)
     u8 = synth.make_filterbank(w)
     d = _delays_for(w)
     rows = [0, 1, 15, 16, 31, 32, 63, 64, 69]
@@ -158,7 +159,7 @@ def test_long_series_use_the_integer_phase_variant(F, oracle_c, kernel):
     with _plan_for(F, w) as plan:
         _set_kernel(F, plan, kernel)
         got = _run(F, plan, u8, "time")[rows]
-    parity.assert_rows(got, ref, "time", f"nfft 2^22/{kernel}")
+    parity.assert_rows(got, ref, "time", f"nfft 2^{log2n}/{kernel}")
 
 
 def test_non_uniform_dm_list_and_kdm_override(F):
