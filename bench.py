@@ -49,7 +49,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="config4",
-                    choices=["tiny", "config2", "config3", "config4", "config5"])
+                    choices=["tiny", "config2", "config3", "config4", "config5", "paper"])
     ap.add_argument("--ndm", type=int, default=None, help="trial DMs (config 4 sweep point)")
     ap.add_argument("--kernel", default="auto",
                     choices=["auto", "generic", "symmetric", "symmetric2"])

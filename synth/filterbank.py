@@ -124,6 +124,16 @@ def workload(name: str, ndm: Optional[int] = None) -> Workload:
         pulses = _pulse_train(period, nsamps, 26.8, 8.0, 6.0, phase0=100.0)
         return Workload("config5", 1005, 400, 110.0, 190.0, tsamp, nsamps, dms, "fourier",
                         tuple(pulses))
+    if name == "paper":
+        # The shape of the paper's own runs: 5 min of 64 us samples (4 687 500,
+        # zero padded to 2^23), 1024 channels over 400 MHz below 1581 MHz, trial DMs 0, 2, 4, ...
+        # The data themselves (simulated signals) were never published: seeded noise + pulses.
+        nsamps, f_lo, f_hi, tsamp = 4687500, 1181.0, 1581.0, 64e-6
+        n = 1024 if ndm is None else int(ndm)
+        dms = tuple(2.0 * i for i in range(n))
+        pulses = _seeded_pulses(1006, 5, nsamps, 0.0, 2.0 * (n - 1), 4.0, 40.0)
+        return Workload("paper_5min", 1006, 1024, f_lo, f_hi, tsamp, nsamps, dms, "time",
+                        tuple(pulses))
     raise KeyError(name)
 
 

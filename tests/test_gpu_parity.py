@@ -327,6 +327,22 @@ def test_full_size_config5_fourier(F, oracle_c):
 
 
 @pytest.mark.slow
+def test_paper_series_length_zero_padded(F, oracle_c):
+    """The paper's series (4 687 500 samples of 64 us, zero padded to 2^23) in its band
+    (1181-1581 MHz, trial DMs 0, 2, 4, ...), 16 of the 1024 channels: padding, the scaled FP64
+    phases (nfft = 2^23) and the padded C2R path at full length."""
+    w = synth.small_workload(1006, 16, 4687500, 128, f_lo=1181.0, f_hi=1581.0, dm_step=2.0)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = [0, 1, 31, 32, 95, 96, 127]
+    ref = O.fdd_rows(u8, d, rows, mode="time")
+    with _plan_for(F, w) as plan:
+        assert plan.nfft == 1 << 23 and plan.get_info()[5] == F.FDD_KERNEL_SYMMETRIC2
+        got = _run(F, plan, u8, "time")[rows]
+    parity.assert_rows(got, ref, "time", "paper series length")
+
+
+@pytest.mark.slow
 def test_full_size_integer_delays(F):
     """P3 at 1024 channels x 2^20 samples: no FFT anywhere in the reference."""
     import torch
