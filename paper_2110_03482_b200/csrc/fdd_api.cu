@@ -47,7 +47,8 @@ struct fdd_plan {
     int device = 0;
     float offset = 0.f;                  // subtracted by a2, restored in bin 0 by a4 (S21)
     // device buffers
-    float2* X = nullptr;                 // [nchans][xpitch]; also the real rows of the in-place R2C
+    float2* X = nullptr;                 // [nchans][xpitch] spectra
+    float* xreal = nullptr;              // [nchans][nfft] unpacked series (out-of-place R2C input)
     long long xpitch = 0;
     float2* Y = nullptr;                 // TIME mode: [y_rows][ypitch] (lazily allocated)
     long long ypitch = 0;
@@ -187,14 +188,15 @@ int build_tables(fdd_plan* p)
 
 int make_fft_plans(fdd_plan* p)
 {
-    // R2C, in place: real rows of pitch 2*xpitch floats, complex rows of pitch xpitch.
+    // R2C, out of place (cuFFT's in-place form adds a packing pass: 6.8 vs 5.1 ms at 1024 x 2^20):
+    // real rows of pitch nfft floats in xreal, complex rows of pitch xpitch in X.
     size_t ws_r2c = 0;
     if (cufftCreate(&p->r2c) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     p->have_r2c = true;
     if (cufftSetAutoAllocation(p->r2c, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     long long n[1] = {p->nfft};
-    long long inembed[1] = {2 * p->xpitch}, onembed[1] = {p->xpitch};
-    if (cufftMakePlanMany64(p->r2c, 1, n, inembed, 1, 2 * p->xpitch, onembed, 1, p->xpitch,
+    long long inembed[1] = {p->nfft}, onembed[1] = {p->xpitch};
+    if (cufftMakePlanMany64(p->r2c, 1, n, inembed, 1, p->nfft, onembed, 1, p->xpitch,
                             CUFFT_R2C, p->nchans, &ws_r2c) != CUFFT_SUCCESS)
         return FDD_ERR_CUFFT;
     p->fft_ws_bytes = ws_r2c;
@@ -273,6 +275,7 @@ void destroy_plan(fdd_plan* p)
     if (p->have_c2r) cufftDestroy(p->c2r);
     if (p->have_c2r_tail) cufftDestroy(p->c2r_tail);
     cudaFree(p->X);
+    cudaFree(p->xreal);
     cudaFree(p->Y);
     cudaFree(p->phase64);
     cudaFree(p->fft_ws);
@@ -299,6 +302,8 @@ int create_common(fdd_plan* p)
     p->xpitch = round_up(p->nbins, kPitchAlign);
     p->ndm_pad = (int)round_up(p->ndm, fdd::kGenDT);
     int rc = dev_alloc(p, &p->X, (size_t)p->nchans * p->xpitch);
+    if (rc != FDD_OK) return rc;
+    rc = dev_alloc(p, &p->xreal, (size_t)p->nchans * p->nfft);
     if (rc != FDD_OK) return rc;
     rc = dev_alloc(p, &p->phase64, (size_t)p->nchans * p->ndm_pad);
     if (rc != FDD_OK) return rc;
@@ -351,14 +356,14 @@ int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
 {
     dim3 grid((unsigned)((p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile),
               (unsigned)((p->nchans + fdd::kUnpackTile - 1) / fdd::kUnpackTile));
-    float* xf = reinterpret_cast<float*>(p->X);
+    float* xf = p->xreal;
     const bool vec = (p->nchans % 4 == 0) && ((uintptr_t)in_u8 % 4 == 0);
     if (vec)
         fdd::k_unpack_transpose<4><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        2 * p->xpitch, p->offset);
+                                                        p->nfft, p->offset);
     else
         fdd::k_unpack_transpose<1><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        2 * p->xpitch, p->offset);
+                                                        p->nfft, p->offset);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
@@ -438,8 +443,7 @@ int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer&
     if (rc != FDD_OK) return rc;
     tm.begin(FDD_STAGE_R2C, 1);
     if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    float* xf = reinterpret_cast<float*>(p->X);
-    if (cufftExecR2C(p->r2c, xf, p->X) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    if (cufftExecR2C(p->r2c, p->xreal, p->X) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     tm.end();
     return FDD_OK;
 }
