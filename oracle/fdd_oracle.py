@@ -228,6 +228,43 @@ def naive_irdft(Y: np.ndarray, nfft: int, nsamps: int, block: int = 256) -> np.n
     return out
 
 
+# ----------------------------------------------------------------------------- O5' (next row f3)
+def naive_irdft_reduced(Y: np.ndarray, nfft: int, nsamps: int, log2_factor: int,
+                        block: int = 256) -> np.ndarray:
+    """Down-sampling "by reducing the length of the inverse Fourier transform" (PAPER.md:98).
+
+    The spectrum is cut at the new Nyquist bin, M = nfft / 2^m points instead of nfft:
+        y_m[n] = (1/nfft) [Re Y_0 + 2 sum_{k=1}^{M/2-1} Re(Y_k e^{2 pi i k n / M}) + Re(Y_{M/2}) (-1)^n]
+    for n < ceil(nsamps / 2^m): the ideal low-pass of the full-rate series y sampled every 2^m
+    samples, in the units of y (scaling 1/nfft as in O5; only Re of the two edge bins, S8).
+    """
+    Y = np.asarray(Y, dtype=np.complex128)
+    n, m = int(nfft), int(log2_factor)
+    M = n >> m
+    assert m >= 0 and M >= 2 and Y.shape[-1] >= M // 2 + 1
+    nout = -(-int(nsamps) // (1 << m))
+    k = np.arange(1, M // 2, dtype=np.int64)
+    out = np.empty(Y.shape[:-1] + (nout,), dtype=np.float64)
+    for n0 in range(0, nout, block):
+        t = np.arange(n0, min(n0 + block, nout), dtype=np.int64)
+        ang = (2.0 * np.pi / M) * ((k[:, None] * t[None, :]) % M)
+        cr, sn = np.cos(ang), np.sin(ang)
+        mid = 2.0 * (Y[..., 1:M // 2].real @ cr - Y[..., 1:M // 2].imag @ sn)
+        sign = np.where(t % 2 == 0, 1.0, -1.0)
+        out[..., n0:n0 + t.size] = (Y[..., :1].real + mid + Y[..., M // 2:M // 2 + 1].real * sign) / n
+    return out
+
+
+def irfft_reduced(Y: np.ndarray, nfft: int, nsamps: int, log2_factor: int) -> np.ndarray:
+    """At-scale tier of naive_irdft_reduced (numpy fp64 FFT; validated against it in the pins)."""
+    n, m = int(nfft), int(log2_factor)
+    M = n >> m
+    nout = -(-int(nsamps) // (1 << m))
+    Yt = np.array(np.asarray(Y, dtype=np.complex128)[..., :M // 2 + 1])
+    # numpy's irfft normalises by 1/M; the definition above by 1/nfft
+    return np.fft.irfft(Yt, n=M, axis=-1)[..., :nout] * (M / n)
+
+
 # ----------------------------------------------------------------------------- whole path
 def fdd_naive(in_u8: np.ndarray, delays: np.ndarray, mode: str = "time") -> np.ndarray:
     """O1..O6 with literal O(N^2) transforms.  Small inputs only (N <= 8192)."""
@@ -252,7 +289,7 @@ def fdd_fft(in_u8: np.ndarray, delays: np.ndarray, mode: str = "time") -> np.nda
 
 
 def fdd_rows(in_u8: np.ndarray, delays: np.ndarray, rows: Iterable[int], mode: str = "time",
-             chan_block: int = 32) -> np.ndarray:
+             chan_block: int = 32, log2_factor: int = 0) -> np.ndarray:
     """At-scale tier for a subset of DM rows, channel block by channel block (memory-light).
 
     Same O1..O6 as fdd_fft; only the loop order differs (channels outermost) so that a
@@ -268,6 +305,10 @@ def fdd_rows(in_u8: np.ndarray, delays: np.ndarray, rows: Iterable[int], mode: s
         c1 = min(c0 + chan_block, nchans)
         X = np.fft.rfft(unpack(in_u8[:, c0:c1], n), axis=-1)
         phase_rotate_sum_c(X, d[:, c0:c1], n, out=Y, accumulate=True)
+    if log2_factor:
+        if mode == "fourier":
+            return Y[..., :(n >> log2_factor) // 2 + 1]
+        return irfft_reduced(Y, n, nsamps, log2_factor)
     if mode == "fourier":
         return Y
     return np.fft.irfft(Y, n=n, axis=-1)[..., :nsamps]

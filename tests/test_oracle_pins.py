@@ -49,6 +49,50 @@ def test_p1_naive_inverse_is_irfft():
     assert np.abs(O.naive_irdft(Y, n, 300) - ref[:, :300]).max() <= 1e-12
 
 
+# ---------------------------------------------------------------- P11: reduced-length inverse
+@pytest.mark.parametrize("m", [0, 1, 3])
+def test_p11_reduced_inverse_samples_a_band_limited_series(m):
+    """PAPER.md:98.  A series whose spectrum stops below the new Nyquist bin M/2 is sampled
+    exactly: y_m[n] = y[n 2^m] (periodic sampling theorem); the series is written as explicit
+    cosines, so the expected values contain no transform at all."""
+    n, M = 1024, 1024 >> m
+    ks = np.array([0, 1, 5, M // 2 - 1][:4 if M // 2 - 1 > 5 else 2])
+    amp = np.array([3.0, 1.5, -0.7, 2.2])[:ks.size]
+    pha = np.array([0.0, 0.3, -1.1, 2.0])[:ks.size]
+    t = np.arange(n)
+    y = sum(a * np.cos(2 * np.pi * k * t / n + p) for a, k, p in zip(amp, ks, pha))
+    Y = O.naive_rdft(y[None, :])
+    got = O.naive_irdft_reduced(Y, n, n, m)[0]
+    assert got.shape == (M,)
+    assert np.abs(got - y[::1 << m]).max() <= 1e-11
+    if m == 0:
+        assert np.abs(got - O.naive_irdft(Y, n, n)[0]).max() <= 1e-12
+
+
+def test_p11_reduced_inverse_is_dirichlet_lowpass_then_sampling():
+    """Brute force in the time domain on a tiny random series: y_m[n] = sum_l y[l] D(n 2^m - l),
+    D the periodic sinc of the kept band |k| <= M/2 (edge bins at half weight, textbook form
+    sin(pi M u / N) / tan(pi u / N) / N); and the two tiers agree."""
+    n, m = 64, 2
+    M = n >> m
+    y = RNG.standard_normal(n)
+    Y = O.naive_rdft(y[None, :])
+    got = O.naive_irdft_reduced(Y, n, n, m)[0]
+    ref = np.zeros(M)
+    for i in range(M):
+        for l in range(n):
+            u = (i << m) - l
+            if u % n == 0:
+                ker = M / n
+            else:
+                ker = math.sin(math.pi * M * u / n) / math.tan(math.pi * u / n) / n
+            ref[i] += y[l] * ker
+    assert np.abs(got - ref).max() <= 1e-12
+    Yc = RNG.standard_normal((3, n // 2 + 1)) + 1j * RNG.standard_normal((3, n // 2 + 1))
+    assert np.abs(O.irfft_reduced(Yc, n, 50, m) - O.naive_irdft_reduced(Yc, n, 50, m)).max() <= 1e-12
+    assert O.irfft_reduced(Yc, n, 50, m).shape == (3, 13)          # ceil(50 / 4)
+
+
 # ---------------------------------------------------------------- O3: delay law, Eq. 1
 def test_delay_law_closed_values():
     # hand-evaluated Eq. 1: K * DM * (nu^-2 - nu0^-2) / tsamp
