@@ -53,6 +53,9 @@ def parse_args():
     ap.add_argument("--ndm", type=int, default=None, help="trial DMs (config 4 sweep point)")
     ap.add_argument("--kernel", default="auto",
                     choices=["auto", "generic", "symmetric", "symmetric2"])
+    ap.add_argument("--decimate", type=int, default=0, metavar="M",
+                    help="row f3: reduced-length inverse transform, output down-sampled by 2^M "
+                         "(PAPER.md:98); the rate still counts the INPUT samples dedispersed")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -245,9 +248,13 @@ def run_b200(args, rank: int, local_rank: int, world: int):
                      "symmetric": F.FDD_KERNEL_SYMMETRIC,
                      "symmetric2": F.FDD_KERNEL_SYMMETRIC2}[args.kernel])
     nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
+    if args.decimate:
+        plan.set_decimation(args.decimate)
+    ns_out, nbins = plan.output_shape()                   # = (nsamps, nbins) at full rate
+    nfft_out = nfft >> args.decimate
     d_in = torch.from_numpy(u8).cuda()
     if mode == F.FDD_MODE_TIME:
-        out = torch.empty((w.ndm, w.nsamps), dtype=torch.float32, device="cuda")
+        out = torch.empty((w.ndm, ns_out), dtype=torch.float32, device="cuda")
     else:
         out = torch.empty((w.ndm, nbins, 2), dtype=torch.float32, device="cuda")
     flush = None
@@ -322,7 +329,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     achieved = FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")   # from the committed ncu summaries
-    if os.path.exists(tpath):
+    if os.path.exists(tpath) and not args.decimate:
         key = f"{w.name}/{w.ndm}/kernel{kernel}"
         for ln in open(tpath):
             f = ln.strip().split(",")
@@ -355,7 +362,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": workload_config(w, world),
+        "config": dict(workload_config(w, world), decimation_log2=args.decimate),
         "clocks": sampler.summary(),
         "e2e": e2e,
         "gpu_launches": int((launches["unpack"] + launches["rotate_sum"])),
@@ -375,8 +382,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     pitch = 2 * ((nbins + 15) // 16 * 16)
     stage_bytes = {
         "unpack": w.nchans * w.nsamps + 4.0 * w.nchans * nfft,
-        "r2c": 4.0 * w.nchans * nfft + 8.0 * w.nchans * nbins,
-        "c2r": (8.0 * w.ndm * nbins + 4.0 * w.ndm * nfft) if mode == F.FDD_MODE_TIME else 0.0,
+        "r2c": 4.0 * w.nchans * nfft + 8.0 * w.nchans * (nfft // 2 + 1),
+        "c2r": (8.0 * w.ndm * nbins + 4.0 * w.ndm * nfft_out) if mode == F.FDD_MODE_TIME else 0.0,
     }
     line["hbm_stages"] = {
         k: {"algorithmic_gb": b * 1e-9, "gbs": b * 1e-9 / (line["stage_ms_per_step"][k] * 1e-3),

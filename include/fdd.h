@@ -97,6 +97,22 @@ int fdd_plan_create_from_delays(fdd_plan **plan_out, int nchans, long long nsamp
  * device (it re-uploads tables the previous execute may still be reading). */
 int fdd_plan_set_kdm(fdd_plan *plan, double k_dm);
 
+/* Down-sampling by a reduced-length inverse transform ("this down-sampling can be
+ * efficiently implemented by reducing the length of the inverse Fourier transform").  With
+ * log2_factor = m > 0 every trial DM is formed only up to the new Nyquist bin nfft / 2^(m+1), so
+ * step a4 does 2^-m of the work, and step a5 is an inverse transform of nfft / 2^m points:
+ *   TIME    rows of ceil(nsamps / 2^m) floats: the ideal low-pass of the full-rate series sampled
+ *           every 2^m samples, in the same units (scaled by 1 / nfft)
+ *   FOURIER rows of nfft / 2^(m+1) + 1 float2: the first bins of the full spectrum
+ * (fdd_plan_get_output_shape gives both lengths).  Meant for the high-DM plans of a search, where
+ * dispersive smearing exceeds 2^m samples.  m = 0 restores full rate.  Requires nfft / 2^m >= 4.
+ * Synchronises the device and drops the TIME-mode scratch, which the next execute re-creates. */
+int fdd_plan_set_decimation(fdd_plan *plan, int log2_factor);
+
+/* Elements per output row: TIME floats (nsamps_out) and FOURIER float2 (nbins_out).  Either pointer
+ * may be NULL. */
+int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long long *nbins_out);
+
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
  * for a delay table that is not in arithmetic progression within every 32-DM tile, or
  * FDD_KERNEL_SYMMETRIC2 for one whose step changes inside a 64-DM tile pair.  AUTO takes the

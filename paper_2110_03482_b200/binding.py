@@ -21,6 +21,7 @@ STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r")
 
 EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
+    "fdd_plan_set_decimation", "fdd_plan_get_output_shape",
     "fdd_execute", "fdd_execute_host", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_error_string",
@@ -59,6 +60,9 @@ def load_library() -> ctypes.CDLL:
                                       P(ctypes.c_size_t), P(c_int)]
     lib.fdd_plan_get_delays.argtypes = [vp, P(c_dbl)]
     lib.fdd_plan_set_profiling.argtypes = [vp, c_int]
+    lib.fdd_plan_set_decimation.argtypes = [vp, c_int]
+    lib.fdd_plan_get_output_shape.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong),
+                                              ctypes.POINTER(ctypes.c_longlong)]
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
     lib.fdd_plan_get_spectrum.argtypes = [vp, P(vp), P(c_ll), P(c_dbl)]
     lib.fdd_rotate_sum_only.argtypes = [vp, vp, c_int, vp]
@@ -174,6 +178,18 @@ class Plan:
         _check(load_library().fdd_plan_get_delays(
             self._h, d.ctypes.data_as(ctypes.POINTER(ctypes.c_double))), "fdd_plan_get_delays")
         return d
+
+    def set_decimation(self, log2_factor: int) -> None:
+        """Reduced-length inverse transform = down-sampling by 2^log2_factor."""
+        _check(load_library().fdd_plan_set_decimation(self._h, int(log2_factor)),
+               "fdd_plan_set_decimation")
+
+    def output_shape(self) -> Tuple[int, int]:
+        """(floats per TIME row, float2 per FOURIER row) after set_decimation."""
+        a, b = ctypes.c_longlong(), ctypes.c_longlong()
+        _check(load_library().fdd_plan_get_output_shape(self._h, ctypes.byref(a), ctypes.byref(b)),
+               "fdd_plan_get_output_shape")
+        return int(a.value), int(b.value)
 
     def set_profiling(self, enable: bool) -> None:
         _check(load_library().fdd_plan_set_profiling(self._h, int(bool(enable))),

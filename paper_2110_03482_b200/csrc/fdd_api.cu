@@ -38,6 +38,10 @@ struct fdd_plan {
     // problem
     int nchans = 0, ndm = 0;
     long long nsamps = 0, nfft = 0, nbins = 0;
+    // output side: reduced-length inverse FFT (fdd_plan_set_decimation); = input side
+    // sizes when log2_dec == 0
+    int log2_dec = 0;
+    long long nfft_out = 0, nbins_out = 0, nsamps_out = 0;
     double tsamp = 0, f_lo = 0, f_hi = 0, kdm = kDefaultKdm;
     bool from_delays = false;
     std::vector<double> dm_list;
@@ -207,11 +211,11 @@ int make_c2r_plan(fdd_plan* p, cufftHandle* h, int batch, size_t* ws)
 {
     if (cufftCreate(h) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     if (cufftSetAutoAllocation(*h, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    long long n[1] = {p->nfft};
-    const bool direct = (p->nsamps == p->nfft);     // straight into the caller's rows
+    long long n[1] = {p->nfft_out};
+    const bool direct = (p->nsamps_out == p->nfft_out);     // straight into the caller's rows
     long long inembed[1] = {p->ypitch};
-    long long onembed[1] = {direct ? p->nfft : 2 * p->ypitch};
-    const long long odist = direct ? p->nfft : 2 * p->ypitch;
+    long long onembed[1] = {direct ? p->nfft_out : 2 * p->ypitch};
+    const long long odist = direct ? p->nfft_out : 2 * p->ypitch;
     if (cufftMakePlanMany64(*h, 1, n, inembed, 1, p->ypitch, onembed, 1, odist, CUFFT_C2R, batch,
                             ws) != CUFFT_SUCCESS)
         return FDD_ERR_CUFFT;
@@ -223,7 +227,7 @@ int make_c2r_plan(fdd_plan* p, cufftHandle* h, int batch, size_t* ws)
 int ensure_time_resources(fdd_plan* p)
 {
     if (p->Y) return FDD_OK;
-    p->ypitch = round_up(p->nbins, kPitchAlign);
+    p->ypitch = round_up(p->nbins_out, kPitchAlign);
     const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
     long long rows = (long long)(kYBudgetBytes / row_bytes);
     size_t free_b = 0, total_b = 0;
@@ -297,6 +301,7 @@ int create_common(fdd_plan* p)
     p->nfft = 2;
     while (p->nfft < p->nsamps) p->nfft <<= 1;
     p->nbins = p->nfft / 2 + 1;
+    p->nfft_out = p->nfft; p->nbins_out = p->nbins; p->nsamps_out = p->nsamps;
     // Without zero padding a constant offset lives in bin 0 alone; with padding it would not.
     p->offset = p->nsamps == p->nfft ? 128.f : 0.f;
     p->xpitch = round_up(p->nbins, kPitchAlign);
@@ -382,19 +387,19 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
         const long long cost3 = (long long)((ntl + 2) / 3) * 315, cost2 = (long long)((ntl + 1) / 2) * 232;
         if (cost3 <= cost2)
-            return fdd::sym2_launch<3, 2>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+            return fdd::sym2_launch<3, 2>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                           rows, dst, opitch, scale, real_edges, dc_add, s);
-        return fdd::sym2_launch<2, 3>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin,
+        return fdd::sym2_launch<2, 3>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                       rows, dst, opitch, scale, real_edges, dc_add, s);
     }
     if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)
-        return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins, p->ndm, j_begin, rows,
+        return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
-    const long long n_kt = (p->nbins + fdd::kGenThreads - 1) / fdd::kGenThreads;
+    const long long n_kt = (p->nbins_out + fdd::kGenThreads - 1) / fdd::kGenThreads;
     if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
     fdd::k_rotate_sum_generic<<<(unsigned)(n_jt * n_kt), fdd::kGenThreads, 0, s>>>(
-        p->X, p->xpitch, p->phase64, p->ndm_pad, p->nchans, p->nbins, j_begin + rows, j_begin, n_jt,
+        p->X, p->xpitch, p->phase64, p->ndm_pad, p->nchans, p->nbins_out, j_begin + rows, j_begin, n_jt,
         dst, opitch, scale, real_edges, dc_add);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
@@ -402,7 +407,7 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
 int launch_c2r_rows(fdd_plan* p, int rows, float2* ysrc, float* dst, cudaStream_t s, int* launches)
 {
     // ysrc: [rows][ypitch]; dst: caller rows (pitch nsamps).
-    const bool direct = (p->nsamps == p->nfft);
+    const bool direct = (p->nsamps_out == p->nfft_out);
     int done = 0;
     while (done < rows) {
         int left = rows - done;
@@ -414,15 +419,15 @@ int launch_c2r_rows(fdd_plan* p, int rows, float2* ysrc, float* dst, cudaStream_
         if (cufftSetStream(h, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
         float2* src = ysrc + (long long)done * p->ypitch;
         if (direct) {
-            if (cufftExecC2R(h, src, dst + (long long)done * p->nsamps) != CUFFT_SUCCESS)
+            if (cufftExecC2R(h, src, dst + (long long)done * p->nsamps_out) != CUFFT_SUCCESS)
                 return FDD_ERR_CUFFT;
             ++*launches;
         } else {
             if (cufftExecC2R(h, src, reinterpret_cast<float*>(src)) != CUFFT_SUCCESS)
                 return FDD_ERR_CUFFT;
-            if (cudaMemcpy2DAsync(dst + (long long)done * p->nsamps, (size_t)p->nsamps * sizeof(float),
+            if (cudaMemcpy2DAsync(dst + (long long)done * p->nsamps_out, (size_t)p->nsamps_out * sizeof(float),
                                   src, (size_t)p->ypitch * sizeof(float2),
-                                  (size_t)p->nsamps * sizeof(float), b, cudaMemcpyDeviceToDevice,
+                                  (size_t)p->nsamps_out * sizeof(float), b, cudaMemcpyDeviceToDevice,
                                   s) != cudaSuccess)
                 return FDD_ERR_CUDA;
             *launches += 2;
@@ -460,8 +465,8 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         for (int j0 = 0; j0 < p->ndm; j0 += step) {
             const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
             tm.begin(FDD_STAGE_ROTATE_SUM, 1);
-            int rc = launch_rotate_sum(p, j0, rows, static_cast<float2*>(out) + (long long)j0 * p->nbins,
-                                       p->nbins, mode, s);
+            int rc = launch_rotate_sum(p, j0, rows, static_cast<float2*>(out) + (long long)j0 * p->nbins_out,
+                                       p->nbins_out, mode, s);
             tm.end();
             if (rc != FDD_OK) return rc;
             chunk_done(j0, rows);
@@ -479,7 +484,7 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         if (rc != FDD_OK) return rc;
         int nl = 0;
         tm.begin(FDD_STAGE_C2R, 0);
-        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + (long long)j0 * p->nsamps, s,
+        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + (long long)j0 * p->nsamps_out, s,
                              &nl);
         tm.end();
         p->launches[FDD_STAGE_C2R] += nl;
@@ -550,6 +555,36 @@ int fdd_plan_set_kdm(fdd_plan* p, double k_dm)
     return build_tables(p);
 }
 
+int fdd_plan_set_decimation(fdd_plan* p, int log2_factor)
+{
+    if (check_plan(p) != FDD_OK || log2_factor < 0 || log2_factor > 30 || (p->nfft >> log2_factor) < 4)
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
+    // the TIME-mode resources depend on the output length: drop them, they are re-made lazily
+    if (p->have_c2r) { cufftDestroy(p->c2r); p->have_c2r = false; }
+    if (p->have_c2r_tail) { cufftDestroy(p->c2r_tail); p->have_c2r_tail = false; }
+    if (p->Y) {
+        cudaFree(p->Y);
+        p->scratch_bytes -= (size_t)p->y_rows * p->ypitch * sizeof(float2);
+        p->Y = nullptr;
+    }
+    p->c2r_tail_batch = 0;
+    p->log2_dec = log2_factor;
+    p->nfft_out = p->nfft >> log2_factor;
+    p->nbins_out = p->nfft_out / 2 + 1;
+    p->nsamps_out = (p->nsamps + (1LL << log2_factor) - 1) >> log2_factor;
+    return FDD_OK;
+}
+
+int fdd_plan_get_output_shape(const fdd_plan* p, long long* nsamps_out, long long* nbins_out)
+{
+    if (!p) return FDD_ERR_INVALID_ARG;
+    if (nsamps_out) *nsamps_out = p->nsamps_out;
+    if (nbins_out) *nbins_out = p->nbins_out;
+    return FDD_OK;
+}
+
 int fdd_plan_set_kernel(fdd_plan* p, int kernel)
 {
     if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
@@ -585,7 +620,7 @@ int fdd_rotate_sum_only(fdd_plan* p, void* out, int mode, void* cuda_stream)
     StageTimer tm(p, s);
     tm.begin(FDD_STAGE_ROTATE_SUM, 1);
     // FOURIER layout (pitch nbins) for either mode: `out` must hold ndm * nbins float2.
-    int rc = launch_rotate_sum(p, 0, p->ndm, static_cast<float2*>(out), p->nbins, mode, s);
+    int rc = launch_rotate_sum(p, 0, p->ndm, static_cast<float2*>(out), p->nbins_out, mode, s);
     tm.end();
     return rc;
 }
@@ -600,8 +635,8 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
     if (!g.ok) return FDD_ERR_CUDA;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t in_bytes = (size_t)p->nsamps * p->nchans;
-    const size_t row_bytes = mode == FDD_MODE_TIME ? (size_t)p->nsamps * sizeof(float)
-                                                   : (size_t)p->nbins * sizeof(float2);
+    const size_t row_bytes = mode == FDD_MODE_TIME ? (size_t)p->nsamps_out * sizeof(float)
+                                                   : (size_t)p->nbins_out * sizeof(float2);
     const size_t out_bytes = row_bytes * p->ndm;
     int rc;
     if (!p->stage_in && (rc = dev_alloc(p, &p->stage_in, in_bytes)) != FDD_OK) return rc;

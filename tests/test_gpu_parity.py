@@ -162,6 +162,44 @@ def test_long_series_phase_variants(F, oracle_c, log2n, kernel):
     parity.assert_rows(got, ref, "time", f"nfft 2^{log2n}/{kernel}")
 
 
+# ------------------------------------------------------------------ row f3: reduced-length inverse
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("nsamps,m", [(8192, 1), (8192, 3), (6000, 2)])
+def test_decimated_outputs_against_the_reduced_inverse_oracle(F, oracle_c, nsamps, m, kernel):
+    """fdd_plan_set_decimation: TIME rows = reduced-length inverse transform,
+    FOURIER rows = the first bins of the full spectrum; m = 0 afterwards restores full rate."""
+    import torch
+    w = synth.small_workload(500 + m, 48, nsamps, 100, dm_step=0.8)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = list(range(w.ndm))
+    ref_t = O.fdd_rows(u8, d, rows, mode="time", log2_factor=m)
+    ref_f = O.fdd_rows(u8, d, rows, mode="fourier", log2_factor=m)
+    d_in = torch.from_numpy(u8).cuda()
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        plan.set_decimation(m)
+        ns_out, nb_out = plan.output_shape()
+        assert ns_out == -(-nsamps // (1 << m)) and nb_out == (plan.nfft >> m) // 2 + 1
+        assert ref_t.shape == (w.ndm, ns_out) and ref_f.shape == (w.ndm, nb_out)
+        out_t = torch.full((w.ndm, ns_out), float("nan"), dtype=torch.float32, device="cuda")
+        out_f = torch.full((w.ndm, nb_out, 2), float("nan"), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out_t, F.FDD_MODE_TIME)
+        plan.execute(d_in, out_f, F.FDD_MODE_FOURIER)
+        torch.cuda.synchronize()
+        got_t = out_t.cpu().numpy()
+        o = out_f.cpu().numpy()
+        got_f = o[..., 0] + 1j * o[..., 1]
+        parity.assert_rows(got_t, ref_t, "time", f"decimated 2^{m}/{kernel}")
+        parity.assert_rows(got_f, ref_f, "fourier", f"decimated 2^{m}/{kernel}")
+        plan.set_decimation(0)
+        full = _run(F, plan, u8, "time")
+    parity.assert_rows(full, O.fdd_rows(u8, d, rows, mode="time"), "time", "full rate again")
+    with pytest.raises(F.FddError):
+        with _plan_for(F, w) as plan:
+            plan.set_decimation(40)
+
+
 def test_non_uniform_dm_list_and_kdm_override(F):
     rng = np.random.default_rng(5)
     dms = np.sort(rng.uniform(0, 300, size=45))
