@@ -24,6 +24,7 @@ constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
 constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
 constexpr int kC2RBatch = 128;                        // rows per cuFFT C2R call (bounds workspace)
 constexpr int kHostChunkRows = 3 * kC2RBatch;         // fdd_execute_host: DM rows per pipelined chunk
+constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
@@ -456,16 +457,21 @@ int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer&
 // Stages a4+a5 from the spectra in p->X.  chunk_done (optional) is called after each DM chunk
 // has been queued, with (j_begin, rows), so fdd_execute_host can overlap the copy back.
 // chunk_rows > 0 caps the DM rows per chunk (multiple of kC2RBatch), for copy/compute overlap.
-template <class F>
+// ring_rows > 0 (a multiple of chunk_rows): `out` is a ring of that many rows, DM row j lands in
+// ring row j % ring_rows, and chunk_begin(j_begin) is called before a chunk's work is queued so
+// the caller can make the stream wait until the ring slot has been drained.
+template <class F, class G>
 int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F chunk_done,
-             int chunk_rows = 0)
+             int chunk_rows, int ring_rows, G chunk_begin)
 {
+    auto out_row = [&](int j0) { return (long long)(ring_rows > 0 ? j0 % ring_rows : j0); };
     if (mode == FDD_MODE_FOURIER) {
         const int step = chunk_rows > 0 ? chunk_rows : p->ndm;
         for (int j0 = 0; j0 < p->ndm; j0 += step) {
             const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
+            chunk_begin(j0);
             tm.begin(FDD_STAGE_ROTATE_SUM, 1);
-            int rc = launch_rotate_sum(p, j0, rows, static_cast<float2*>(out) + (long long)j0 * p->nbins_out,
+            int rc = launch_rotate_sum(p, j0, rows, static_cast<float2*>(out) + out_row(j0) * p->nbins_out,
                                        p->nbins_out, mode, s);
             tm.end();
             if (rc != FDD_OK) return rc;
@@ -478,13 +484,14 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
     const int step = (chunk_rows > 0 && chunk_rows < p->y_rows) ? chunk_rows : p->y_rows;
     for (int j0 = 0; j0 < p->ndm; j0 += step) {
         const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
+        chunk_begin(j0);
         tm.begin(FDD_STAGE_ROTATE_SUM, 1);
         rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s);
         tm.end();
         if (rc != FDD_OK) return rc;
         int nl = 0;
         tm.begin(FDD_STAGE_C2R, 0);
-        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + (long long)j0 * p->nsamps_out, s,
+        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + out_row(j0) * p->nsamps_out, s,
                              &nl);
         tm.end();
         p->launches[FDD_STAGE_C2R] += nl;
@@ -607,7 +614,7 @@ int fdd_execute(fdd_plan* p, const unsigned char* in_u8, void* out, int mode, vo
     StageTimer tm(p, s);
     int rc = run_pre(p, in_u8, s, tm);
     if (rc != FDD_OK) return rc;
-    return run_post(p, out, mode, s, tm, [](int, int) {});
+    return run_post(p, out, mode, s, tm, [](int, int) {}, 0, 0, [](int) {});
 }
 
 int fdd_rotate_sum_only(fdd_plan* p, void* out, int mode, void* cuda_stream)
@@ -637,8 +644,14 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
     const size_t in_bytes = (size_t)p->nsamps * p->nchans;
     const size_t row_bytes = mode == FDD_MODE_TIME ? (size_t)p->nsamps_out * sizeof(float)
                                                    : (size_t)p->nbins_out * sizeof(float2);
-    const size_t out_bytes = row_bytes * p->ndm;
+    // The device side of the output is a ring of kHostRingChunks chunks (Algorithm 1's output
+    // buffers): results may be larger than HBM, only the host array holds them all.
     int rc;
+    if (mode == FDD_MODE_TIME && (rc = ensure_time_resources(p)) != FDD_OK) return rc;
+    // chunk = what run_post will step by: kHostChunkRows, or the whole Y scratch if that is smaller
+    const int chunk = (mode == FDD_MODE_TIME && p->y_rows < kHostChunkRows) ? p->y_rows : kHostChunkRows;
+    const int ring_rows = kHostRingChunks * chunk;
+    const size_t out_bytes = row_bytes * (size_t)(p->ndm < ring_rows ? p->ndm : ring_rows);
     if (!p->stage_in && (rc = dev_alloc(p, &p->stage_in, in_bytes)) != FDD_OK) return rc;
     if (p->stage_out_bytes < out_bytes) {
         if (p->stage_out) { cudaFree(p->stage_out); p->scratch_bytes -= p->stage_out_bytes; p->stage_out = nullptr; }
@@ -655,25 +668,39 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
     StageTimer tm(p, s);
     rc = run_pre(p, p->stage_in, s, tm);
     if (rc != FDD_OK) return rc;
-    size_t ev_used = 0;
+    // two events per chunk: [2i] results ready (on s), [2i+1] copied back (on copy_stream)
+    const int nchunks = (p->ndm + chunk - 1) / chunk;
+    while (p->chunk_events.size() < (size_t)2 * nchunks) {
+        cudaEvent_t e;
+        if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            return FDD_ERR_CUDA;
+        }
+        p->chunk_events.push_back(e);
+    }
     bool copy_fail = false;
+    // a ring slot is rewritten only after the chunk that used it last has been copied back
+    auto chunk_begin = [&](int j0) {
+        const int i = j0 / chunk;
+        if (i >= kHostRingChunks &&
+            cudaStreamWaitEvent(s, p->chunk_events[2 * (i - kHostRingChunks) + 1], 0) != cudaSuccess)
+            copy_fail = true;
+    };
     // Algorithm 1 lines 19-22: copy each finished DM chunk back while later chunks still compute.
     auto chunk_done = [&](int j0, int rows) {
-        if (ev_used == p->chunk_events.size()) {
-            cudaEvent_t e;
-            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { copy_fail = true; return; }
-            p->chunk_events.push_back(e);
-        }
-        cudaEvent_t e = p->chunk_events[ev_used++];
-        if (cudaEventRecord(e, s) != cudaSuccess || cudaStreamWaitEvent(p->copy_stream, e, 0) != cudaSuccess ||
+        const int i = j0 / chunk;
+        cudaEvent_t ready = p->chunk_events[2 * i], copied = p->chunk_events[2 * i + 1];
+        if (cudaEventRecord(ready, s) != cudaSuccess ||
+            cudaStreamWaitEvent(p->copy_stream, ready, 0) != cudaSuccess ||
             cudaMemcpyAsync(static_cast<char*>(out_host) + (size_t)j0 * row_bytes,
-                            static_cast<char*>(p->stage_out) + (size_t)j0 * row_bytes,
+                            static_cast<char*>(p->stage_out) + (size_t)(j0 % ring_rows) * row_bytes,
                             (size_t)rows * row_bytes, cudaMemcpyDeviceToHost,
-                            p->copy_stream) != cudaSuccess)
+                            p->copy_stream) != cudaSuccess ||
+            cudaEventRecord(copied, p->copy_stream) != cudaSuccess)
             copy_fail = true;
     };
     // DM chunks of kHostChunkRows rows: the copy back of chunk i overlaps the compute of chunk i+1
-    rc = run_post(p, p->stage_out, mode, s, tm, chunk_done, kHostChunkRows);
+    rc = run_post(p, p->stage_out, mode, s, tm, chunk_done, chunk, ring_rows, chunk_begin);
     if (rc != FDD_OK) return rc;
     if (copy_fail) { cudaGetLastError(); return FDD_ERR_CUDA; }
     if (cudaStreamSynchronize(p->copy_stream) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
