@@ -56,6 +56,9 @@ def parse_args():
     ap.add_argument("--decimate", type=int, default=0, metavar="M",
                     help="row f3: reduced-length inverse transform, output down-sampled by 2^M "
                          "(PAPER.md:98); the rate still counts the INPUT samples dedispersed")
+    ap.add_argument("--with-tdd", action="store_true",
+                    help="row f4: also time the time-domain comparator (fdd_tdd_execute) on the "
+                         "same input and report it as tdd_comparator")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -296,6 +299,29 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     units = float(w.ndm) * w.nsamps * world               # DM-trials x samples, all ranks
     value = units / (ms_step * 1e-3)
 
+    # ---- the time-domain comparator on the same input (row f4; not part of `value`) -----
+    tdd = None
+    if args.with_tdd and mode == F.FDD_MODE_TIME and not args.decimate:
+        for _ in range(2):
+            plan.tdd_execute(d_in, out, stream)
+        torch.cuda.synchronize()
+        plan.set_profiling(True)
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record(stream)
+        for _ in range(args.steps):
+            plan.tdd_execute(d_in, out, stream)
+        t1.record(stream)
+        torch.cuda.synchronize()
+        tms = t0.elapsed_time(t1) / args.steps
+        st, _ = plan.get_stage_ms()
+        plan.set_profiling(False)
+        tdd = {"what": "time-domain shift-and-add (Eq. 2) on the same input, same GPU: "
+                       "fdd_tdd_execute = u8 transpose + integer shift-and-add",
+               "ms_per_step": tms, "value": float(w.ndm) * w.nsamps / (tms * 1e-3), "unit": UNIT,
+               "stage_ms_per_step": {"tdd_transpose": st["tdd_transpose"] / args.steps,
+                                     "tdd_shift_add": st["tdd_shift_add"] / args.steps},
+               "fdd_over_tdd_time": ms_step / tms}
+
     # ---- end to end through the host-buffer entry point ---------------------------------
     e2e = None
     if not args.no_e2e:
@@ -363,11 +389,13 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": dict(workload_config(w, world), decimation_log2=args.decimate),
+        "tdd_comparator": tdd,
         "clocks": sampler.summary(),
         "e2e": e2e,
         "gpu_launches": int((launches["unpack"] + launches["rotate_sum"])),
         "library_calls": int(launches["r2c"] + launches["c2r"]),
-        "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+        "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()
+                              if not k.startswith("tdd_")},
         "roofline": roofline,
         "plan": {"nfft": nfft, "nbins": nbins, "valid_len": valid, "max_delay_samples": maxd,
                  "scratch_bytes": scratch, "kernel": kernel},

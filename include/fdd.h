@@ -73,7 +73,8 @@ enum fdd_kernel {
 /* Stage indices for fdd_plan_get_stage_ms. */
 enum fdd_stage {
     FDD_STAGE_UNPACK = 0, FDD_STAGE_R2C = 1, FDD_STAGE_ROTATE_SUM = 2, FDD_STAGE_C2R = 3,
-    FDD_NUM_STAGES = 4
+    FDD_STAGE_TDD_TRANSPOSE = 4, FDD_STAGE_TDD_SHIFT_ADD = 5,     /* fdd_tdd_execute only */
+    FDD_NUM_STAGES = 6
 };
 
 /* a1. Create a plan for nchans channels whose centres run evenly from f_lo_mhz (channel 0) to
@@ -154,6 +155,16 @@ int fdd_plan_get_info(const fdd_plan *plan, long long *nfft, long long *nbins,
 
 /* Copy the plan's delay table to delay_samples_host[ndm][nchans] (HOST). */
 int fdd_plan_get_delays(const fdd_plan *plan, double *delay_samples_host);
+
+/* The time-domain comparator (the paper's "TDD"; Eq. 2) for the same
+ * plan, on the same GPU: out[j][n] = sum_c in[(n + s[j][c]) mod nsamps][c], with the plan's delays
+ * rounded to the nearest sample, s = floor(d + 1/2).  Exact integer sums, written as float32.
+ *   in_u8  DEVICE, uint8 [nsamps][nchans] as for fdd_execute
+ *   out    DEVICE, float [ndm][nsamps]; the first valid_len samples of a row are free of wrap-around
+ * Asynchronous on cuda_stream.  Ignores fdd_plan_set_kernel / fdd_plan_set_decimation.  It exists
+ * to put the paper's comparison (FDD against optimised time-domain dedispersion) on one machine;
+ * it is not a step of the FDD path. */
+int fdd_tdd_execute(fdd_plan *plan, const unsigned char *in_u8, float *out, void *cuda_stream);
 
 /* Stage timing.  fdd_plan_set_profiling(plan, 1) makes every following execute record CUDA
  * events between the stages on its stream, and zeroes the totals; fdd_plan_get_stage_ms waits

@@ -16,13 +16,13 @@ LIB_PATH = os.path.join(HERE, "csrc", "libfdd_b200.so")
 FDD_MODE_TIME, FDD_MODE_FOURIER = 0, 1
 FDD_KERNEL_AUTO, FDD_KERNEL_GENERIC, FDD_KERNEL_SYMMETRIC, FDD_KERNEL_SYMMETRIC2 = 0, 1, 2, 3
 FDD_OK = 0
-FDD_NUM_STAGES = 4
-STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r")
+FDD_NUM_STAGES = 6
+STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift_add")
 
 EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
     "fdd_plan_set_decimation", "fdd_plan_get_output_shape",
-    "fdd_execute", "fdd_execute_host", "fdd_plan_destroy", "fdd_plan_get_info",
+    "fdd_execute", "fdd_execute_host", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_error_string",
 )
@@ -55,6 +55,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_set_kernel.argtypes = [vp, c_int]
     lib.fdd_execute.argtypes = [vp, vp, vp, c_int, vp]
     lib.fdd_execute_host.argtypes = [vp, vp, vp, c_int, vp]
+    lib.fdd_tdd_execute.argtypes = [vp, vp, vp, vp]
     lib.fdd_plan_destroy.argtypes = [vp]
     lib.fdd_plan_get_info.argtypes = [vp, P(c_ll), P(c_ll), P(c_ll), P(c_dbl),
                                       P(ctypes.c_size_t), P(c_int)]
@@ -158,6 +159,11 @@ class Plan:
         """Host buffers in/out; returns when the result has landed in ``out_host``."""
         _check(load_library().fdd_execute_host(self._h, _ptr(in_host), _ptr(out_host), int(mode),
                                                _stream_handle(stream)), "fdd_execute_host")
+
+    def tdd_execute(self, in_u8, out, stream=None) -> None:
+        """The time-domain comparator (Eq. 2): device tensors, out float32 [ndm][nsamps]."""
+        _check(load_library().fdd_tdd_execute(self._h, _ptr(in_u8), _ptr(out),
+                                              _stream_handle(stream)), "fdd_tdd_execute")
 
     def rotate_sum_only(self, out, mode: int = FDD_MODE_FOURIER, stream=None) -> None:
         _check(load_library().fdd_rotate_sum_only(self._h, _ptr(out), int(mode),

@@ -16,6 +16,7 @@
 #include "fdd_kernels_pre.cuh"
 #include "fdd_kernels_sym.cuh"
 #include "fdd_kernels_sym2.cuh"
+#include "fdd_kernels_tdd.cuh"
 
 namespace {
 
@@ -80,7 +81,11 @@ struct fdd_plan {
     bool profiling = false;
     std::vector<StageEvent> events;
     size_t events_used = 0;
-    int launches[FDD_NUM_STAGES] = {0, 0, 0, 0};
+    int launches[FDD_NUM_STAGES] = {0, 0, 0, 0, 0, 0};
+    // time-domain comparator (fdd_tdd_execute), built on first use
+    unsigned char* tdd_xt = nullptr;     // [nchans][tdd_tpitch] transposed bytes, periodic tail
+    long long tdd_tpitch = 0;
+    int* tdd_shifts = nullptr;           // [nchans][ndm_pad] shifts mod nsamps
     size_t scratch_bytes = 0;
 };
 
@@ -281,6 +286,8 @@ void destroy_plan(fdd_plan* p)
     if (p->have_c2r_tail) cufftDestroy(p->c2r_tail);
     cudaFree(p->X);
     cudaFree(p->xreal);
+    cudaFree(p->tdd_xt);
+    cudaFree(p->tdd_shifts);
     cudaFree(p->Y);
     cudaFree(p->phase64);
     cudaFree(p->fft_ws);
@@ -559,6 +566,12 @@ int fdd_plan_set_kdm(fdd_plan* p, double k_dm)
     if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
     p->kdm = k_dm;
     build_delays(p);
+    // the comparator's shift table follows the delays: drop it, it is rebuilt on next use
+    if (p->tdd_shifts) {
+        cudaFree(p->tdd_shifts); cudaFree(p->tdd_xt);
+        p->scratch_bytes -= (size_t)p->nchans * p->ndm_pad * sizeof(int) + (size_t)p->nchans * p->tdd_tpitch;
+        p->tdd_shifts = nullptr; p->tdd_xt = nullptr;
+    }
     return build_tables(p);
 }
 
@@ -708,6 +721,51 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
         return FDD_ERR_CUDA;
     }
     return FDD_OK;
+}
+
+int fdd_tdd_execute(fdd_plan* p, const unsigned char* in_u8, float* out, void* cuda_stream)
+{
+    if (check_plan(p) != FDD_OK || !in_u8 || !out) return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    int rc;
+    if (!p->tdd_shifts) {
+        // Eq. 2: shifts rounded to the nearest sample, reduced mod nsamps (the result is circular)
+        std::vector<int> sh((size_t)p->nchans * p->ndm_pad, 0);
+        long long smax = 0;
+        for (int j = 0; j < p->ndm; ++j)
+            for (int c = 0; c < p->nchans; ++c) {
+                long long v = (long long)floor(p->delays[(size_t)j * p->nchans + c] + 0.5) % p->nsamps;
+                if (v < 0) v += p->nsamps;
+                sh[(size_t)c * p->ndm_pad + j] = (int)v;
+                if (v > smax) smax = v;
+            }
+        if (p->nsamps > 2147483647LL - 256) return FDD_ERR_UNSUPPORTED;
+        p->tdd_tpitch = round_up(p->nsamps + smax + 128, 64);
+        if ((rc = dev_alloc(p, &p->tdd_shifts, sh.size())) != FDD_OK) return rc;
+        if ((rc = dev_alloc(p, &p->tdd_xt, (size_t)p->nchans * p->tdd_tpitch)) != FDD_OK) return rc;
+        if (cudaMemcpy(p->tdd_shifts, sh.data(), sh.size() * sizeof(int), cudaMemcpyHostToDevice) !=
+            cudaSuccess) {
+            cudaGetLastError();
+            return FDD_ERR_CUDA;
+        }
+    }
+    StageTimer tm(p, s);
+    tm.begin(FDD_STAGE_TDD_TRANSPOSE, 1);
+    dim3 tgrid((unsigned)(p->tdd_tpitch / 64), (unsigned)((p->nchans + 63) / 64));
+    fdd::k_tdd_transpose<<<tgrid, 256, 0, s>>>(in_u8, p->tdd_xt, p->nchans, p->nsamps, p->tdd_tpitch);
+    tm.end();
+    if (cudaGetLastError() != cudaSuccess) return FDD_ERR_CUDA;
+    const int ntiles_dm = (p->ndm + fdd::kTddDms - 1) / fdd::kTddDms;
+    const long long ntb = (p->nsamps + fdd::kTddTile - 1) / fdd::kTddTile;
+    if ((long long)ntiles_dm * ntb > 2147483647LL) return FDD_ERR_UNSUPPORTED;
+    tm.begin(FDD_STAGE_TDD_SHIFT_ADD, 1);
+    fdd::k_tdd_shift_add<<<(unsigned)(ntiles_dm * ntb), fdd::kTddWarps * 32, 0, s>>>(
+        p->tdd_xt, p->tdd_tpitch, p->tdd_shifts, p->ndm_pad, p->nchans, p->nsamps, p->ndm, ntiles_dm,
+        out);
+    tm.end();
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
 int fdd_plan_destroy(fdd_plan* p)
