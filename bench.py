@@ -365,7 +365,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     # sym2 111 FFMA2 per 96 DMs (NS = 3) or 79 per 64 (NS = 2, the library's choice when that
     # leaves fewer 32-DM sub-tiles idle), sym 47 FFMA2 per 32 DMs, generic 4 FFMA per element
     ntl = (w.ndm + 31) // 32
-    ns3 = ((ntl + 2) // 3) * 315 <= ((ntl + 1) // 2) * 232
+    ns3 = ((ntl + 2) // 3) * 294 <= ((ntl + 1) // 2) * 232
     kname, fma_lanes = {F.FDD_KERNEL_SYMMETRIC2: ("k_rotate_sum_sym2<%d>" % (3 if ns3 else 2),
                                                   111 * 2 / 96.0 if ns3 else 79 * 2 / 64.0),
                         F.FDD_KERNEL_SYMMETRIC: ("k_rotate_sum_sym", 47 * 2 / 32.0)}.get(

@@ -391,9 +391,9 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
     if (p->kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
         // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of
-        // one group per (channel, warp): 315 cycles for NS = 3, 232 for NS = 2
+        // one group per (channel, warp): 294 cycles for NS = 3, 232 for NS = 2
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
-        const long long cost3 = (long long)((ntl + 2) / 3) * 315, cost2 = (long long)((ntl + 1) / 2) * 232;
+        const long long cost3 = (long long)((ntl + 2) / 3) * 294, cost2 = (long long)((ntl + 1) / 2) * 232;
         if (cost3 <= cost2)
             return fdd::sym2_launch<3, 2>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                           rows, dst, opitch, scale, real_edges, dc_add, s);
