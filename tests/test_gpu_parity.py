@@ -297,6 +297,35 @@ def test_execute_host_output_ring_wraps(F):
             assert np.array_equal(got[:384], dev[:384])
 
 
+def test_streams_determinism_and_plan_churn(F):
+    """Executes on a non-default stream, repeated executes are bit-identical (no atomics, fixed
+    summation order), and creating / destroying plans gives the device memory back."""
+    import torch
+    w = synth.small_workload(33, 96, 4096, 200, dm_step=0.3)
+    u8 = synth.make_filterbank(w)
+    d_in = torch.from_numpy(u8).cuda()
+    free0 = None
+    first = None
+    for it in range(6):
+        with _plan_for(F, w) as plan:
+            out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                plan.execute(d_in, out, F.FDD_MODE_TIME, st)
+                plan.execute(d_in, out, F.FDD_MODE_TIME, st)
+            st.synchronize()
+            got = out.cpu().numpy()
+            del out
+        if first is None:
+            first = got
+        assert np.array_equal(got, first)
+        torch.cuda.synchronize()
+        torch.cuda.empty_cache()
+        if free0 is None:                  # after the first plan: cuFFT and kernel modules are loaded
+            free0 = torch.cuda.mem_get_info()[0]
+    assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)
+
+
 def test_stage_profile_and_errors(F):
     import torch
     w = synth.small_workload(32, 16, 1024, 8)
