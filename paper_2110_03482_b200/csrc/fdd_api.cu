@@ -66,8 +66,12 @@ struct fdd_plan {
     int kernel = FDD_KERNEL_GENERIC;     // resolved choice
     int kernel_request = FDD_KERNEL_AUTO;
     // FFT
-    cufftHandle r2c = 0, c2r = 0, c2r_tail = 0;
-    bool have_r2c = false, have_c2r = false, have_c2r_tail = false;
+    cufftHandle r2c = 0;
+    bool have_r2c = false;
+    // a5 plans in two families: [0] C2R of nfft_out points from Y; [1] C2C of nfft_out/2 points from
+    // the pre-twiddled Z the mirrored sym2 epilogue writes (fdd_kernels_sym2.cuh, kMirror)
+    cufftHandle c2r[2] = {0, 0}, c2r_tail[2] = {0, 0};
+    bool have_c2r[2] = {false, false}, have_c2r_tail[2] = {false, false};
     int c2r_batch = 0, c2r_tail_batch = 0;
     void* fft_ws = nullptr;
     size_t fft_ws_bytes = 0;
@@ -213,67 +217,86 @@ int make_fft_plans(fdd_plan* p)
     return FDD_OK;
 }
 
-int make_c2r_plan(fdd_plan* p, cufftHandle* h, int batch, size_t* ws)
+int make_c2r_plan(fdd_plan* p, int family, cufftHandle* h, int batch, size_t* ws)
 {
     if (cufftCreate(h) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     if (cufftSetAutoAllocation(*h, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    long long n[1] = {p->nfft_out};
     const bool direct = (p->nsamps_out == p->nfft_out);     // straight into the caller's rows
     long long inembed[1] = {p->ypitch};
-    long long onembed[1] = {direct ? p->nfft_out : 2 * p->ypitch};
-    const long long odist = direct ? p->nfft_out : 2 * p->ypitch;
-    if (cufftMakePlanMany64(*h, 1, n, inembed, 1, p->ypitch, onembed, 1, odist, CUFFT_C2R, batch,
-                            ws) != CUFFT_SUCCESS)
-        return FDD_ERR_CUFFT;
+    if (family == 0) {
+        long long n[1] = {p->nfft_out};
+        long long onembed[1] = {direct ? p->nfft_out : 2 * p->ypitch};
+        const long long odist = direct ? p->nfft_out : 2 * p->ypitch;
+        if (cufftMakePlanMany64(*h, 1, n, inembed, 1, p->ypitch, onembed, 1, odist, CUFFT_C2R, batch,
+                                ws) != CUFFT_SUCCESS)
+            return FDD_ERR_CUFFT;
+    } else {
+        // nfft_out / 2 complex points; the output pairs are the even / odd real samples
+        long long n[1] = {p->nfft_out / 2};
+        long long onembed[1] = {direct ? p->nfft_out / 2 : p->ypitch};
+        const long long odist = direct ? p->nfft_out / 2 : p->ypitch;
+        if (cufftMakePlanMany64(*h, 1, n, inembed, 1, p->ypitch, onembed, 1, odist, CUFFT_C2C, batch,
+                                ws) != CUFFT_SUCCESS)
+            return FDD_ERR_CUFFT;
+    }
     return FDD_OK;
 }
 
 // TIME-mode resources are allocated on the first TIME execute (a FOURIER-only plan such as
 // config 5 never needs the 16 GiB of Y).
-int ensure_time_resources(fdd_plan* p)
+int ensure_time_resources(fdd_plan* p, int family = 0)
 {
-    if (p->Y) return FDD_OK;
-    p->ypitch = round_up(p->nbins_out, kPitchAlign);
-    const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
-    long long rows = (long long)(kYBudgetBytes / row_bytes);
-    size_t free_b = 0, total_b = 0;
-    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
-        long long fit = (long long)(free_b / 2 / row_bytes);
-        if (fit < rows) rows = fit;
-    }
-    if (rows >= p->ndm) rows = p->ndm;
-    else rows = rows >= 3 * kC2RBatch ? rows / (3 * kC2RBatch) * (3 * kC2RBatch)   // whole 96-DM groups
-                                      : rows / kC2RBatch * kC2RBatch;
-    if (rows < 1) return FDD_ERR_ALLOC;
-    p->y_rows = (int)rows;
-    p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
-    size_t ws_a = 0, ws_b = 0;
-    int rc = make_c2r_plan(p, &p->c2r, p->c2r_batch, &ws_a);
-    p->have_c2r = true;
-    if (rc != FDD_OK) return rc;
-    // tails: of a full Y chunk and of the last (short) chunk; at most one distinct tail size is
-    // planned, any other remainder is issued row by row through it.
-    const int last_rows = p->ndm % p->y_rows ? p->ndm % p->y_rows : p->y_rows;
-    int tail = last_rows % p->c2r_batch;
-    if (tail == 0) tail = p->y_rows % p->c2r_batch;
-    if (tail) {
-        rc = make_c2r_plan(p, &p->c2r_tail, tail, &ws_b);
-        p->have_c2r_tail = true;
-        if (rc != FDD_OK) return rc;
+    int rc;
+    if (!p->Y) {
+        p->ypitch = round_up(p->nbins_out, kPitchAlign);
+        const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
+        long long rows = (long long)(kYBudgetBytes / row_bytes);
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+            long long fit = (long long)(free_b / 2 / row_bytes);
+            if (fit < rows) rows = fit;
+        }
+        if (rows >= p->ndm) rows = p->ndm;
+        else rows = rows >= 3 * kC2RBatch ? rows / (3 * kC2RBatch) * (3 * kC2RBatch)   // whole 96-DM groups
+                                          : rows / kC2RBatch * kC2RBatch;
+        if (rows < 1) return FDD_ERR_ALLOC;
+        p->y_rows = (int)rows;
+        p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
+        // tails: of a full Y chunk and of the last (short) chunk; at most one distinct tail size
+        const int last_rows = p->ndm % p->y_rows ? p->ndm % p->y_rows : p->y_rows;
+        int tail = last_rows % p->c2r_batch;
+        if (tail == 0) tail = p->y_rows % p->c2r_batch;
         p->c2r_tail_batch = tail;
+        if ((rc = dev_alloc(p, &p->Y, (size_t)p->y_rows * p->ypitch)) != FDD_OK) return rc;
     }
-    size_t need = ws_a > ws_b ? ws_a : ws_b;
+    if (p->have_c2r[family]) return FDD_OK;
+    size_t ws_a = 0, ws_b = 0;
+    rc = make_c2r_plan(p, family, &p->c2r[family], p->c2r_batch, &ws_a);
+    p->have_c2r[family] = true;
+    if (rc != FDD_OK) return rc;
+    if (p->c2r_tail_batch) {
+        rc = make_c2r_plan(p, family, &p->c2r_tail[family], p->c2r_tail_batch, &ws_b);
+        p->have_c2r_tail[family] = true;
+        if (rc != FDD_OK) return rc;
+    }
+    const size_t need = ws_a > ws_b ? ws_a : ws_b;
     if (need > p->fft_ws_bytes) {
+        // (no execute is in flight on a plan that is being grown: plans are not re-entrant)
+        if (cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
         if (p->fft_ws) { cudaFree(p->fft_ws); p->scratch_bytes -= p->fft_ws_bytes; p->fft_ws = nullptr; }
-        p->fft_ws_bytes = need;
+        p->fft_ws_bytes = 0;
         rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->fft_ws), need);
         if (rc != FDD_OK) return rc;
-        if (cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+        p->fft_ws_bytes = need;
     }
-    if (cufftSetWorkArea(p->c2r, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    if (p->have_c2r_tail && cufftSetWorkArea(p->c2r_tail, p->fft_ws) != CUFFT_SUCCESS)
-        return FDD_ERR_CUFFT;
-    return dev_alloc(p, &p->Y, (size_t)p->y_rows * p->ypitch);
+    // every plan works in the one shared area (never two transforms in flight)
+    if (cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    for (int f = 0; f < 2; ++f) {
+        if (p->have_c2r[f] && cufftSetWorkArea(p->c2r[f], p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+        if (p->have_c2r_tail[f] && cufftSetWorkArea(p->c2r_tail[f], p->fft_ws) != CUFFT_SUCCESS)
+            return FDD_ERR_CUFFT;
+    }
+    return FDD_OK;
 }
 
 void destroy_plan(fdd_plan* p)
@@ -282,8 +305,10 @@ void destroy_plan(fdd_plan* p)
     DeviceGuard g(p->device);
     cudaDeviceSynchronize();
     if (p->have_r2c) cufftDestroy(p->r2c);
-    if (p->have_c2r) cufftDestroy(p->c2r);
-    if (p->have_c2r_tail) cufftDestroy(p->c2r_tail);
+    for (int f = 0; f < 2; ++f) {
+        if (p->have_c2r[f]) cufftDestroy(p->c2r[f]);
+        if (p->have_c2r_tail[f]) cufftDestroy(p->c2r_tail[f]);
+    }
     cudaFree(p->X);
     cudaFree(p->xreal);
     cudaFree(p->tdd_xt);
@@ -381,8 +406,10 @@ int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
 }
 
 // a4 on DM rows [j_begin, j_begin + rows) into dst (row pitch opitch float2).
+// mirror (SYMMETRIC2, TIME mode only): dst receives the pre-twiddled Z of the half-length inverse
+// transform instead of Y (fdd_kernels_sym2.cuh).
 int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
-                      cudaStream_t s)
+                      cudaStream_t s, bool mirror = false)
 {
     const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
     const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
@@ -395,9 +422,9 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
         const long long cost3 = (long long)((ntl + 2) / 3) * 294, cost2 = (long long)((ntl + 1) / 2) * 232;
         if (cost3 <= cost2)
-            return fdd::sym2_launch<3, 2>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
+            return fdd::sym2_launch<3, 2>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                           rows, dst, opitch, scale, real_edges, dc_add, s);
-        return fdd::sym2_launch<2, 3>(p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
+        return fdd::sym2_launch<2, 3>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                       rows, dst, opitch, scale, real_edges, dc_add, s);
     }
     if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)
@@ -412,7 +439,8 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
-int launch_c2r_rows(fdd_plan* p, int rows, float2* ysrc, float* dst, cudaStream_t s, int* launches)
+int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst, cudaStream_t s,
+                    int* launches)
 {
     // ysrc: [rows][ypitch]; dst: caller rows (pitch nsamps).
     const bool direct = (p->nsamps_out == p->nfft_out);
@@ -421,17 +449,21 @@ int launch_c2r_rows(fdd_plan* p, int rows, float2* ysrc, float* dst, cudaStream_
         int left = rows - done;
         cufftHandle h;
         int b;
-        if (left >= p->c2r_batch) { h = p->c2r; b = p->c2r_batch; }
-        else if (p->have_c2r_tail && left >= p->c2r_tail_batch) { h = p->c2r_tail; b = p->c2r_tail_batch; }
+        if (left >= p->c2r_batch) { h = p->c2r[family]; b = p->c2r_batch; }
+        else if (p->have_c2r_tail[family] && left >= p->c2r_tail_batch) { h = p->c2r_tail[family]; b = p->c2r_tail_batch; }
         else return FDD_ERR_UNSUPPORTED;     // cannot happen: tails are planned in ensure_time_resources
         if (cufftSetStream(h, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
         float2* src = ysrc + (long long)done * p->ypitch;
+        float* drow = dst + (long long)done * p->nsamps_out;
         if (direct) {
-            if (cufftExecC2R(h, src, dst + (long long)done * p->nsamps_out) != CUFFT_SUCCESS)
+            if ((family == 0 ? cufftExecC2R(h, src, drow)
+                             : cufftExecC2C(h, src, reinterpret_cast<float2*>(drow), CUFFT_INVERSE)) !=
+                CUFFT_SUCCESS)
                 return FDD_ERR_CUFFT;
             ++*launches;
         } else {
-            if (cufftExecC2R(h, src, reinterpret_cast<float*>(src)) != CUFFT_SUCCESS)
+            if ((family == 0 ? cufftExecC2R(h, src, reinterpret_cast<float*>(src))
+                             : cufftExecC2C(h, src, src, CUFFT_INVERSE)) != CUFFT_SUCCESS)
                 return FDD_ERR_CUFFT;
             if (cudaMemcpy2DAsync(dst + (long long)done * p->nsamps_out, (size_t)p->nsamps_out * sizeof(float),
                                   src, (size_t)p->ypitch * sizeof(float2),
@@ -486,20 +518,22 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         }
         return FDD_OK;
     }
-    int rc = ensure_time_resources(p);
+    // SYMMETRIC2 writes the pre-twiddled spectrum of the half-length complex inverse (family 1)
+    const int family = (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
+    int rc = ensure_time_resources(p, family);
     if (rc != FDD_OK) return rc;
     const int step = (chunk_rows > 0 && chunk_rows < p->y_rows) ? chunk_rows : p->y_rows;
     for (int j0 = 0; j0 < p->ndm; j0 += step) {
         const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
         chunk_begin(j0);
         tm.begin(FDD_STAGE_ROTATE_SUM, 1);
-        rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s);
+        rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s, family == 1);
         tm.end();
         if (rc != FDD_OK) return rc;
         int nl = 0;
         tm.begin(FDD_STAGE_C2R, 0);
-        rc = launch_c2r_rows(p, rows, p->Y, static_cast<float*>(out) + out_row(j0) * p->nsamps_out, s,
-                             &nl);
+        rc = launch_c2r_rows(p, family, rows, p->Y, static_cast<float*>(out) + out_row(j0) * p->nsamps_out,
+                             s, &nl);
         tm.end();
         p->launches[FDD_STAGE_C2R] += nl;
         if (rc != FDD_OK) return rc;
@@ -582,8 +616,10 @@ int fdd_plan_set_decimation(fdd_plan* p, int log2_factor)
     DeviceGuard g(p->device);
     if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
     // the TIME-mode resources depend on the output length: drop them, they are re-made lazily
-    if (p->have_c2r) { cufftDestroy(p->c2r); p->have_c2r = false; }
-    if (p->have_c2r_tail) { cufftDestroy(p->c2r_tail); p->have_c2r_tail = false; }
+    for (int f = 0; f < 2; ++f) {
+        if (p->have_c2r[f]) { cufftDestroy(p->c2r[f]); p->have_c2r[f] = false; }
+        if (p->have_c2r_tail[f]) { cufftDestroy(p->c2r_tail[f]); p->have_c2r_tail[f] = false; }
+    }
     if (p->Y) {
         cudaFree(p->Y);
         p->scratch_bytes -= (size_t)p->y_rows * p->ypitch * sizeof(float2);

@@ -170,7 +170,11 @@ __device__ __forceinline__ void sym2_accumulate(const Sym2Seed<NS>& cur, float2 
     }
 }
 
-template <int NS, int kMinCtas, int kMode>
+// kMirror (TIME mode): a CTA holds 64 bins k and their mirrors N/2 - k, and the epilogue writes
+// Z[k] = (Y[k] + conj Y[N/2-k]) + i e^{2 pi i k / N} (Y[k] - conj Y[N/2-k]) instead of Y: the inverse
+// real transform of N points is then ONE complex transform of N/2 points of Z (its output pairs are
+// the even / odd samples), and cuFFT's own pre-processing pass over Y (a quarter of a5) is gone.
+template <int NS, int kMinCtas, int kMode, bool kMirror>
 __global__ void __launch_bounds__(kSym2Threads, kMinCtas)
 k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   const unsigned long long* __restrict__ centre64,
@@ -188,9 +192,20 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
     // 1-D grid, DM tile-group fastest: CTAs resident together read the same X slab through L2.
     const int gr = (int)(blockIdx.x % (unsigned)ngroups);
     const long long kb = blockIdx.x / (unsigned)ngroups;
-    const long long kraw = kb * kSym2Threads + threadIdx.x;
-    const bool live = kraw < nbins;
-    const long long k = live ? kraw : nbins - 1;      // dead lanes redo the last bin, never stored
+    bool live;
+    long long k;
+    if (kMirror) {
+        constexpr int kHalf = kSym2Threads / 2;
+        const long long H = nbins - 1;                // N/2 (even); pairs (kl, H - kl), kl = 0..H/2
+        const long long kl = kb * kHalf + (threadIdx.x & (kHalf - 1));
+        const bool upper = threadIdx.x >= kHalf;
+        live = upper ? kl < H / 2 : kl <= H / 2;      // the middle bin pairs with itself: lower only
+        k = live ? (upper ? H - kl : kl) : H / 2;     // dead lanes redo the middle bin, never stored
+    } else {
+        const long long kraw = kb * kSym2Threads + threadIdx.x;
+        live = kraw < nbins;
+        k = live ? kraw : nbins - 1;                  // dead lanes redo the last bin, never stored
+    }
     const int tA = tile0 + NS * gr;
 
     float2 U[NS][kSymPairs], V[NS][kSymPairs];
@@ -257,24 +272,67 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
             slot = slot + 1 == kSym2Depth ? 0 : slot + 1;
         }
     }
-    if (!live) return;
-
     const bool edge = real_edges && (k == 0 || k == nbins - 1);
     const float dc = k == 0 ? dc_add : 0.f;           // the mean a2 removed (already scaled)
+    if (!kMirror) {
+        if (!live) return;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            if (tA + s >= ntiles_total) break;        // tail group: computed, not stored
+            const int j0 = (tA + s) * kSymT;
+#pragma unroll
+            for (int m = 0; m < kSymPairs; ++m) {
+                const float2 u = U[s][m], v = V[s][m];
+                const int jp = j0 + kSymPairs + m, jm = j0 + kSymPairs - 1 - m;
+                if (jp < ndm)
+                    out[(long long)(jp - row0) * opitch + k] =
+                        make_float2((u.x - v.y) * scale + dc, edge ? 0.f : (v.x + u.y) * scale);
+                if (jm < ndm)
+                    out[(long long)(jm - row0) * opitch + k] =
+                        make_float2((u.x + v.y) * scale + dc, edge ? 0.f : (v.x - u.y) * scale);
+            }
+        }
+        return;
+    }
+
+    // Mirror epilogue: partners (threads t and t ^ 64) swap their Y through shared memory, 16 rows
+    // at a time, and each writes Z of its own bin (bin N/2 itself has no Z entry).
+    constexpr int kHalf = kSym2Threads / 2;
+    const long long H = nbins - 1;
+    float2* ex = reinterpret_cast<float2*>(s_p);      // [kSymPairs][kSym2Threads], after the loop
+    double wsd, wcd;
+    sincospi((double)k / (double)H, &wsd, &wcd);      // w = e^{2 pi i k / N}, N = 2 H
+    const float ws = (float)wsd, wc = (float)wcd;
+    const bool self = (k == H - k);
+    const bool store = live && k < H;
+    __syncthreads();                                  // everyone is done with s_p
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        if (tA + s >= ntiles_total) break;            // tail group: computed, not stored
+        if (tA + s >= ntiles_total) break;            // tail group (uniform over the CTA)
         const int j0 = (tA + s) * kSymT;
 #pragma unroll
-        for (int m = 0; m < kSymPairs; ++m) {
-            const float2 u = U[s][m], v = V[s][m];
-            const int jp = j0 + kSymPairs + m, jm = j0 + kSymPairs - 1 - m;
-            if (jp < ndm)
-                out[(long long)(jp - row0) * opitch + k] =
-                    make_float2((u.x - v.y) * scale + dc, edge ? 0.f : (v.x + u.y) * scale);
-            if (jm < ndm)
-                out[(long long)(jm - row0) * opitch + k] =
-                    make_float2((u.x + v.y) * scale + dc, edge ? 0.f : (v.x - u.y) * scale);
+        for (int sgn = 0; sgn < 2; ++sgn) {
+            float2 y[kSymPairs];
+#pragma unroll
+            for (int m = 0; m < kSymPairs; ++m) {
+                const float2 u = U[s][m], v = V[s][m];
+                y[m] = sgn == 0 ? make_float2((u.x - v.y) * scale + dc, edge ? 0.f : (v.x + u.y) * scale)
+                                : make_float2((u.x + v.y) * scale + dc, edge ? 0.f : (v.x - u.y) * scale);
+                ex[m * kSym2Threads + threadIdx.x] = y[m];
+            }
+            __syncthreads();
+#pragma unroll
+            for (int m = 0; m < kSymPairs; ++m) {
+                const int j = sgn == 0 ? j0 + kSymPairs + m : j0 + kSymPairs - 1 - m;
+                float2 p = ex[m * kSym2Threads + (threadIdx.x ^ kHalf)];     // Y[N/2 - k]
+                if (self) p = y[m];
+                // A = Y[k], B = conj(Y[N/2 - k]):  Z = (A + B) + i w (A - B)
+                const float sr = y[m].x + p.x, si = y[m].y - p.y;
+                const float dr = y[m].x - p.x, di = y[m].y + p.y;
+                const float2 z = make_float2(sr - (wc * di + ws * dr), si + (wc * dr - ws * di));
+                if (store && j < ndm) out[(long long)(j - row0) * opitch + k] = z;
+            }
+            __syncthreads();
         }
     }
 }
@@ -282,7 +340,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
 // Rows [j_begin, j_begin + rows) -> dst[(j - j_begin) * opitch + k]; j_begin a multiple of kSymT.
 // The sub-tiles of the chunk are grouped NS at a time from its first one.
 template <int NS, int kMinCtas>
-inline int sym2_launch(long long nfft, const SymTables& t, const float2* X, long long xpitch, int nchans,
+inline int sym2_launch(bool mirror, long long nfft, const SymTables& t, const float2* X, long long xpitch, int nchans,
                        long long nbins, int ndm, int j_begin, int rows, float2* dst,
                        long long opitch, float scale, int real_edges, float dc_add, cudaStream_t s)
 {
@@ -292,18 +350,27 @@ inline int sym2_launch(long long nfft, const SymTables& t, const float2* X, long
     const int ngroups = (ntl + NS - 1) / NS;
     const int row_end = j_begin + rows < ndm ? j_begin + rows : ndm;
     const int ntiles_total = tile0 + ntl;             // sub-tiles past this chunk are not touched
-    const long long nkb = (nbins + kSym2Threads - 1) / kSym2Threads;
+    // mirror: 64 bin pairs (k, N/2 - k), k = 0 .. N/4, per CTA
+    const long long nkb = mirror ? ((nbins - 1) / 2 + 1 + kSym2Threads / 2 - 1) / (kSym2Threads / 2)
+                                 : (nbins + kSym2Threads - 1) / kSym2Threads;
     if ((long long)ngroups * nkb > 2147483647LL) return -5;
     int pshift = 0;                                   // FP64-pipe phases: see sym2_phases
     while ((nfft >> pshift) > (1LL << 21)) ++pshift;
     const unsigned grid = (unsigned)(ngroups * nkb);
-#define FDD_SYM2_LAUNCH(MODE)                                                                      \
-    k_rotate_sum_sym2<NS, kMinCtas, MODE><<<grid, kSym2Threads, 0, s>>>(                           \
+#define FDD_SYM2_LAUNCH(MODE, MIRROR)                                                              \
+    k_rotate_sum_sym2<NS, kMinCtas, MODE, MIRROR><<<grid, kSym2Threads, 0, s>>>(                   \
         X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst, \
         opitch, j_begin, scale, real_edges, dc_add, pshift)
-    if (pshift == 0) FDD_SYM2_LAUNCH(0);
-    else if (pshift <= 2) FDD_SYM2_LAUNCH(1);         // nfft <= 2^23; longer: integer phases
-    else FDD_SYM2_LAUNCH(2);
+    const int mode = pshift == 0 ? 0 : (pshift <= 2 ? 1 : 2);   // nfft <= 2^23; longer: integer phases
+    if (mirror) {
+        if (mode == 0) FDD_SYM2_LAUNCH(0, true);
+        else if (mode == 1) FDD_SYM2_LAUNCH(1, true);
+        else FDD_SYM2_LAUNCH(2, true);
+    } else {
+        if (mode == 0) FDD_SYM2_LAUNCH(0, false);
+        else if (mode == 1) FDD_SYM2_LAUNCH(1, false);
+        else FDD_SYM2_LAUNCH(2, false);
+    }
 #undef FDD_SYM2_LAUNCH
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
