@@ -11,11 +11,12 @@
 // bin) the kernel then issues 32 NS accumulate FFMA2 (2 per pair, 16 pairs, NS sub-tiles) but
 // only 15 recurrence FFMA2, and ONE seed (phase products, table and X loads, c2):
 //     NS = 3: 111 FFMA2 per 96 trial DMs = 2.31 FMA lanes per (dm, channel, bin) element,
-//             192 accumulator registers, 244 in all, 2 CTAs x 128 threads per SM;
+//             192 accumulator registers, 254 in all, 2 CTAs x 128 threads per SM;
 //     NS = 2:  79 FFMA2 per 64 trial DMs = 2.47 lanes, 168 registers, 3 CTAs per SM;
 // against 94 FFMA2 per 64 for independent 32-DM tiles.  The recurrence is no longer than before
 // (m <= 15), so the error bound of fdd_kernels_sym.cuh is unchanged.  Measured on B200 at
-// 1024 channels x 2^20 samples x 4096 trial DMs: NS = 3 195 ms, NS = 2 214 ms, 32-DM tiles 333 ms.
+// 1024 channels x 2^20 samples x 4096 trial DMs: NS = 3 183 ms, NS = 2 ~205 ms, 32-DM tiles 333 ms
+// (profiles/r01c_*, r01b_*, r01a_*).
 #pragma once
 #include "fdd_kernels_sym.cuh"
 
