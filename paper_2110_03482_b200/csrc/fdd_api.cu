@@ -23,8 +23,8 @@ namespace {
 constexpr double kDefaultKdm = 4.148808e3;            // MHz^2 pc^-1 cm^3 s (reading S5)
 constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
 constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
-constexpr int kC2RBatch = 128;                        // rows per cuFFT C2R call (bounds workspace)
-constexpr int kHostChunkRows = 3 * kC2RBatch;         // fdd_execute_host: DM rows per pipelined chunk
+constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
+constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
@@ -257,8 +257,8 @@ int ensure_time_resources(fdd_plan* p, int family = 0)
             if (fit < rows) rows = fit;
         }
         if (rows >= p->ndm) rows = p->ndm;
-        else rows = rows >= 3 * kC2RBatch ? rows / (3 * kC2RBatch) * (3 * kC2RBatch)   // whole 96-DM groups
-                                          : rows / kC2RBatch * kC2RBatch;
+        else rows = rows >= kC2RBatch ? rows / kC2RBatch * kC2RBatch          // whole 96-DM groups
+                                      : (rows >= 96 ? rows / 96 * 96 : (rows >= 32 ? 32 : rows));
         if (rows < 1) return FDD_ERR_ALLOC;
         p->y_rows = (int)rows;
         p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
@@ -427,7 +427,9 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         return fdd::sym2_launch<2, 3>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                       rows, dst, opitch, scale, real_edges, dc_add, s);
     }
-    if (p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2)
+    // (a chunk that does not start on a 32-DM tile - only with rows of > 0.75 GiB - goes generic)
+    if ((p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2) &&
+        j_begin % fdd::kSymT == 0)
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
@@ -519,9 +521,13 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         return FDD_OK;
     }
     // SYMMETRIC2 writes the pre-twiddled spectrum of the half-length complex inverse (family 1)
-    const int family = (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
+    int family = (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
     int rc = ensure_time_resources(p, family);
     if (rc != FDD_OK) return rc;
+    if (family == 1 && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0) {
+        family = 0;                          // chunks off the 32-DM tiling run the generic kernel
+        if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
+    }
     const int step = (chunk_rows > 0 && chunk_rows < p->y_rows) ? chunk_rows : p->y_rows;
     for (int j0 = 0; j0 < p->ndm; j0 += step) {
         const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
