@@ -66,8 +66,9 @@ enum fdd_kernel {
     FDD_KERNEL_AUTO = 0,       /* symmetric kernel where the DM grid allows it, else generic     */
     FDD_KERNEL_GENERIC = 1,    /* any delay table: one exactly range-reduced phasor per element  */
     FDD_KERNEL_SYMMETRIC = 2,  /* DM tiles in arithmetic progression: paired +-m rows */
-    FDD_KERNEL_SYMMETRIC2 = 3  /* same, two adjacent 32-DM tiles per CTA sharing one phasor
-                                  recurrence; needs one DM step across each 64-DM tile pair      */
+    FDD_KERNEL_SYMMETRIC2 = 3  /* same, up to three adjacent 32-DM tiles per CTA sharing one phasor
+                                  recurrence; the groups follow the uniform segments of the DM
+                                  plan (a group ends where the DM step changes)                  */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */
@@ -115,9 +116,9 @@ int fdd_plan_set_decimation(fdd_plan *plan, int log2_factor);
 int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long long *nbins_out);
 
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
- * for a delay table that is not in arithmetic progression within every 32-DM tile, or
- * FDD_KERNEL_SYMMETRIC2 for one whose step changes inside a 64-DM tile pair.  AUTO takes the
- * fastest kernel the table allows: SYMMETRIC2, else SYMMETRIC, else GENERIC. */
+ * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
+ * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
+ * allows: SYMMETRIC2 (uniform and piecewise-uniform DM plans), else GENERIC. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 
 /* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy

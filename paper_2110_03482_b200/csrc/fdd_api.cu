@@ -163,7 +163,7 @@ inline unsigned long long cycles_to_fixed64(long double cyc)
 // AUTO: the fastest kernel the delay table allows.
 int resolve_kernel(const fdd_plan* p, int request)
 {
-    const bool sym2_ok = p->sym_ok && p->sym.pair_ok;
+    const bool sym2_ok = p->sym_ok;      // groups of sub-tiles follow the DM plan's uniform segments
     switch (request) {
         case FDD_KERNEL_GENERIC: return FDD_KERNEL_GENERIC;
         case FDD_KERNEL_SYMMETRIC: return p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC;
@@ -420,7 +420,10 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of
         // one group per (channel, warp): 294 cycles for NS = 3, 232 for NS = 2
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
-        const long long cost3 = (long long)((ntl + 2) / 3) * 294, cost2 = (long long)((ntl + 1) / 2) * 232;
+        std::vector<unsigned short> gs;
+        std::vector<unsigned char> gc;
+        const long long cost3 = 294LL * fdd::sym2_group(p->sym, j_begin / fdd::kSymT, ntl, 3, &gs, &gc);
+        const long long cost2 = 232LL * fdd::sym2_group(p->sym, j_begin / fdd::kSymT, ntl, 2, &gs, &gc);
         if (cost3 <= cost2)
             return fdd::sym2_launch<3, 2>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
                                           rows, dst, opitch, scale, real_edges, dc_add, s);
@@ -652,7 +655,7 @@ int fdd_plan_set_kernel(fdd_plan* p, int kernel)
     if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
     if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_SYMMETRIC2) return FDD_ERR_INVALID_ARG;
     if (kernel == FDD_KERNEL_SYMMETRIC && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
-    if (kernel == FDD_KERNEL_SYMMETRIC2 && !(p->sym_ok && p->sym.pair_ok)) return FDD_ERR_UNSUPPORTED;
+    if (kernel == FDD_KERNEL_SYMMETRIC2 && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     p->kernel_request = kernel;
     p->kernel = resolve_kernel(p, kernel);
     return FDD_OK;

@@ -48,27 +48,32 @@ struct SymTables {
     unsigned long long* half64 = nullptr;     // [ntiles][nchans] frac(h_c / nfft) * 2^64
     int ntiles = 0;
     size_t bytes = 0;
-    bool pair_ok = false;   // adjacent sub-tiles continue one progression (fdd_kernels_sym2.cuh)
+    bool pair_ok = false;   // every adjacent pair of sub-tiles continues one progression
+    // cont[t] != 0: sub-tile t + 1 continues the progression of sub-tile t (same half step, centre
+    // 64 half steps on), so the two may share a CTA of fdd_kernels_sym2.cuh; host side only
+    std::vector<unsigned char> cont;
 };
 
-// Do all adjacent sub-tiles t, t+1 continue one arithmetic progression in every channel: same half
-// step, and centre(t+1) = centre(t) + 64 half steps?  (host, plan time; fdd_kernels_sym2.cuh groups
-// two or three adjacent sub-tiles from any chunk start)
-inline bool sym_pairs_share_step(const std::vector<unsigned long long>& centre64,
-                                 const std::vector<unsigned long long>& half64, int ntiles,
-                                 int nchans)
+// For every adjacent pair of sub-tiles t, t+1: do they continue one arithmetic progression in every
+// channel (same half step, centre(t+1) = centre(t) + 64 half steps)?  (host, plan time)
+inline void sym_continuations(const std::vector<unsigned long long>& centre64,
+                              const std::vector<unsigned long long>& half64, int ntiles, int nchans,
+                              std::vector<unsigned char>* cont)
 {
     // units of 2^-64 cycle per bin; bins < 2^31: 2^20 is < 1e-4 cycles of phase anywhere
     auto near0 = [](unsigned long long d) { return d <= (1ULL << 20) || d >= ~0ULL - (1ULL << 20); };
-    for (int t = 0; t + 1 < ntiles; ++t)
-        for (int c = 0; c < nchans; ++c) {
+    cont->assign(ntiles > 0 ? ntiles : 0, 0);
+    for (int t = 0; t + 1 < ntiles; ++t) {
+        bool ok = true;
+        for (int c = 0; c < nchans && ok; ++c) {
             const unsigned long long ha = half64[(size_t)t * nchans + c];
             const unsigned long long hb = half64[(size_t)(t + 1) * nchans + c];
             const unsigned long long ca = centre64[(size_t)t * nchans + c];
             const unsigned long long cb = centre64[(size_t)(t + 1) * nchans + c];
-            if (!near0(ha - hb) || !near0(cb - ca - (ha << 6))) return false;
+            ok = near0(ha - hb) && near0(cb - ca - (ha << 6));
         }
-    return true;
+        (*cont)[t] = ok ? 1 : 0;
+    }
 }
 
 inline void sym_free_tables(SymTables* t)
@@ -79,6 +84,7 @@ inline void sym_free_tables(SymTables* t)
     t->ntiles = 0;
     t->bytes = 0;
     t->pair_ok = false;
+    t->cont.clear();
 }
 
 inline unsigned long long sym_fixed64(long double cyc)
@@ -133,7 +139,9 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
         return -3;
     }
     t->ntiles = ntiles;
-    t->pair_ok = sym_pairs_share_step(hc, hh, ntiles, nchans);
+    sym_continuations(hc, hh, ntiles, nchans, &t->cont);
+    t->pair_ok = true;
+    for (int tl = 0; tl + 1 < ntiles; ++tl) t->pair_ok = t->pair_ok && t->cont[tl];
     t->bytes = 2 * bytes;
     if (scratch_bytes) *scratch_bytes += t->bytes;
     *ok = true;

@@ -171,6 +171,15 @@ __device__ __forceinline__ void sym2_accumulate(const Sym2Seed<NS>& cur, float2 
     }
 }
 
+// The sub-tiles one launch covers, grouped for the CTAs: group g = sub-tiles tile0 + start[g] ...
+// + count[g] - 1 (count <= NS), all continuing one progression.  On a uniform DM grid every group is
+// full; on a piecewise-uniform DM plan a group ends where the DM step changes.  Passed by value.
+constexpr int kSym2MaxGroups = 256;
+struct Sym2Groups {
+    unsigned short start[kSym2MaxGroups];
+    unsigned char count[kSym2MaxGroups];
+};
+
 // kMirror (TIME mode): a CTA holds 64 bins k and their mirrors N/2 - k, and the epilogue writes
 // Z[k] = (Y[k] + conj Y[N/2-k]) + i e^{2 pi i k / N} (Y[k] - conj Y[N/2-k]) instead of Y: the inverse
 // real transform of N points is then ONE complex transform of N/2 points of Z (its output pairs are
@@ -180,7 +189,7 @@ __global__ void __launch_bounds__(kSym2Threads, kMinCtas)
 k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
                   const unsigned long long* __restrict__ centre64,
                   const unsigned long long* __restrict__ half64, int nchans, long long nbins,
-                  int tile0, int ngroups, int ntiles_total, int ndm, float2* __restrict__ out,
+                  int tile0, int ngroups, const Sym2Groups groups, int ndm, float2* __restrict__ out,
                   long long opitch, int row0, float scale, int real_edges, float dc_add,
                   int pshift)
 {
@@ -207,7 +216,8 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
         live = kraw < nbins;
         k = live ? kraw : nbins - 1;                  // dead lanes redo the last bin, never stored
     }
-    const int tA = tile0 + NS * gr;
+    const int tA = tile0 + groups.start[gr];
+    const int nsub = groups.count[gr];                // sub-tiles beyond it are computed, not stored
 
     float2 U[NS][kSymPairs], V[NS][kSymPairs];
 #pragma unroll
@@ -279,7 +289,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
         if (!live) return;
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
-            if (tA + s >= ntiles_total) break;        // tail group: computed, not stored
+            if (s >= nsub) break;
             const int j0 = (tA + s) * kSymT;
 #pragma unroll
             for (int m = 0; m < kSymPairs; ++m) {
@@ -309,7 +319,7 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
     __syncthreads();                                  // everyone is done with s_p
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        if (tA + s >= ntiles_total) break;            // tail group (uniform over the CTA)
+        if (s >= nsub) break;                         // (uniform over the CTA)
         const int j0 = (tA + s) * kSymT;
 #pragma unroll
         for (int sgn = 0; sgn < 2; ++sgn) {
@@ -338,8 +348,24 @@ k_rotate_sum_sym2(const float2* __restrict__ X, long long xpitch,
     }
 }
 
+// Greedy grouping of sub-tiles [tile0, tile0 + ntl) into runs of at most ns that continue one
+// progression; returns the number of groups (starts relative to tile0).
+inline int sym2_group(const SymTables& t, int tile0, int ntl, int ns, std::vector<unsigned short>* start,
+                      std::vector<unsigned char>* count)
+{
+    start->clear();
+    count->clear();
+    for (int i = 0; i < ntl;) {
+        int n = 1;
+        while (n < ns && i + n < ntl && t.cont[tile0 + i + n - 1]) ++n;
+        start->push_back((unsigned short)i);
+        count->push_back((unsigned char)n);
+        i += n;
+    }
+    return (int)start->size();
+}
+
 // Rows [j_begin, j_begin + rows) -> dst[(j - j_begin) * opitch + k]; j_begin a multiple of kSymT.
-// The sub-tiles of the chunk are grouped NS at a time from its first one.
 template <int NS, int kMinCtas>
 inline int sym2_launch(bool mirror, long long nfft, const SymTables& t, const float2* X, long long xpitch, int nchans,
                        long long nbins, int ndm, int j_begin, int rows, float2* dst,
@@ -348,29 +374,39 @@ inline int sym2_launch(bool mirror, long long nfft, const SymTables& t, const fl
     if (j_begin % kSymT != 0 || !t.centre64) return -5;
     const int tile0 = j_begin / kSymT;
     const int ntl = (rows + kSymT - 1) / kSymT;
-    const int ngroups = (ntl + NS - 1) / NS;
+    if (ntl > 65535) return -5;
     const int row_end = j_begin + rows < ndm ? j_begin + rows : ndm;
-    const int ntiles_total = tile0 + ntl;             // sub-tiles past this chunk are not touched
+    std::vector<unsigned short> gstart;
+    std::vector<unsigned char> gcount;
+    const int ngroups_all = sym2_group(t, tile0, ntl, NS, &gstart, &gcount);
     // mirror: 64 bin pairs (k, N/2 - k), k = 0 .. N/4, per CTA
     const long long nkb = mirror ? ((nbins - 1) / 2 + 1 + kSym2Threads / 2 - 1) / (kSym2Threads / 2)
                                  : (nbins + kSym2Threads - 1) / kSym2Threads;
-    if ((long long)ngroups * nkb > 2147483647LL) return -5;
     int pshift = 0;                                   // FP64-pipe phases: see sym2_phases
     while ((nfft >> pshift) > (1LL << 21)) ++pshift;
-    const unsigned grid = (unsigned)(ngroups * nkb);
+    const int mode = pshift == 0 ? 0 : (pshift <= 2 ? 1 : 2);   // nfft <= 2^23; longer: integer phases
 #define FDD_SYM2_LAUNCH(MODE, MIRROR)                                                              \
     k_rotate_sum_sym2<NS, kMinCtas, MODE, MIRROR><<<grid, kSym2Threads, 0, s>>>(                   \
-        X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, ntiles_total, row_end, dst, \
+        X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, groups, row_end, dst,      \
         opitch, j_begin, scale, real_edges, dc_add, pshift)
-    const int mode = pshift == 0 ? 0 : (pshift <= 2 ? 1 : 2);   // nfft <= 2^23; longer: integer phases
-    if (mirror) {
-        if (mode == 0) FDD_SYM2_LAUNCH(0, true);
-        else if (mode == 1) FDD_SYM2_LAUNCH(1, true);
-        else FDD_SYM2_LAUNCH(2, true);
-    } else {
-        if (mode == 0) FDD_SYM2_LAUNCH(0, false);
-        else if (mode == 1) FDD_SYM2_LAUNCH(1, false);
-        else FDD_SYM2_LAUNCH(2, false);
+    for (int g0 = 0; g0 < ngroups_all; g0 += kSym2MaxGroups) {     // one launch per 256 groups
+        const int ngroups = ngroups_all - g0 < kSym2MaxGroups ? ngroups_all - g0 : kSym2MaxGroups;
+        Sym2Groups groups;
+        for (int g = 0; g < kSym2MaxGroups; ++g) {
+            groups.start[g] = g < ngroups ? gstart[g0 + g] : 0;
+            groups.count[g] = g < ngroups ? gcount[g0 + g] : 0;
+        }
+        if ((long long)ngroups * nkb > 2147483647LL) return -5;
+        const unsigned grid = (unsigned)(ngroups * nkb);
+        if (mirror) {
+            if (mode == 0) FDD_SYM2_LAUNCH(0, true);
+            else if (mode == 1) FDD_SYM2_LAUNCH(1, true);
+            else FDD_SYM2_LAUNCH(2, true);
+        } else {
+            if (mode == 0) FDD_SYM2_LAUNCH(0, false);
+            else if (mode == 1) FDD_SYM2_LAUNCH(1, false);
+            else FDD_SYM2_LAUNCH(2, false);
+        }
     }
 #undef FDD_SYM2_LAUNCH
     return cudaGetLastError() == cudaSuccess ? 0 : -3;

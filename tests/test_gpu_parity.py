@@ -217,25 +217,30 @@ def test_non_uniform_dm_list_and_kdm_override(F):
 
 
 def test_kernel_selection_follows_the_dm_grid(F):
-    """AUTO: SYMMETRIC2 on one uniform grid, SYMMETRIC when the step changes between 32-DM tiles
-    (a piecewise-uniform DM plan), GENERIC otherwise; each against the fp64 oracle."""
+    """AUTO: SYMMETRIC2 on a uniform grid AND on a piecewise-uniform DM plan whose step changes
+    between 32-DM tiles (its CTA groups end where the step changes), GENERIC otherwise; each
+    against the fp64 oracle, the piecewise plan also through the 32-DM-tile kernel."""
     w = synth.small_workload(78, 40, 2048, 2)
     u8 = synth.make_filterbank(w)
     uniform = np.arange(96) * 0.75
-    piecewise = np.concatenate([np.arange(32) * 0.5, 16.0 + np.arange(32) * 1.0,
-                                48.0 + np.arange(20) * 2.0])
+    piecewise = np.concatenate([np.arange(32) * 0.5, 16.0 + np.arange(64) * 1.0,
+                                80.0 + np.arange(96) * 2.0, 272.0 + np.arange(20) * 4.0])
     random = np.sort(np.random.default_rng(6).uniform(0, 80, size=70))
-    for dms, want in ((uniform, F.FDD_KERNEL_SYMMETRIC2), (piecewise, F.FDD_KERNEL_SYMMETRIC),
+    for dms, want in ((uniform, F.FDD_KERNEL_SYMMETRIC2), (piecewise, F.FDD_KERNEL_SYMMETRIC2),
                       (random, F.FDD_KERNEL_GENERIC)):
         d = O.delay_table(40, w.f_lo, w.f_hi, w.tsamp, dms)
-        ref = O.fdd_fft(u8, d)
-        with F.Plan.create(40, 2048, w.tsamp, w.f_lo, w.f_hi, dms) as plan:
-            assert plan.get_info()[5] == want
-            if want != F.FDD_KERNEL_SYMMETRIC2:
-                with pytest.raises(F.FddError):
-                    plan.set_kernel(F.FDD_KERNEL_SYMMETRIC2)
-            got = _run(F, plan, u8, "time")
-        parity.assert_rows(got, ref, "time", f"kernel selection {want}")
+        for mode in ("time", "fourier"):
+            ref = O.fdd_fft(u8, d, mode=mode)
+            with F.Plan.create(40, 2048, w.tsamp, w.f_lo, w.f_hi, dms) as plan:
+                assert plan.get_info()[5] == want
+                if want == F.FDD_KERNEL_GENERIC:
+                    with pytest.raises(F.FddError):
+                        plan.set_kernel(F.FDD_KERNEL_SYMMETRIC2)
+                got = _run(F, plan, u8, mode)
+                parity.assert_rows(got, ref, mode, f"kernel selection {want}/{mode}")
+                if dms is piecewise:
+                    plan.set_kernel(F.FDD_KERNEL_SYMMETRIC)
+                    parity.assert_rows(_run(F, plan, u8, mode), ref, mode, "piecewise/32-DM tiles")
 
 
 # ------------------------------------------------------------------ P3 on the GPU: exact integers
