@@ -118,7 +118,9 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
  * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
  * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
- * allows: SYMMETRIC2 (uniform and piecewise-uniform DM plans), else GENERIC. */
+ * allows: SYMMETRIC2 (uniform and piecewise-uniform DM plans), else GENERIC.  A plan whose DM step
+ * changes INSIDE a 32-DM tile is not piecewise-uniform in this sense and runs on the (about five
+ * times slower) generic kernel: make the segments of a DM plan multiples of 32 trial DMs. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 
 /* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy
