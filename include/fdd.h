@@ -119,7 +119,7 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
  * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
  * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
  * allows: SYMMETRIC2 (uniform and piecewise-uniform DM plans), else GENERIC.  A plan whose DM step
- * changes INSIDE a 32-DM tile is not piecewise-uniform in this sense and runs on the (about five
+ * changes INSIDE a 32-DM tile is not piecewise-uniform in this sense and runs on the (about seven
  * times slower) generic kernel: make the segments of a DM plan multiples of 32 trial DMs. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 
