@@ -374,6 +374,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     ns3 = ((ntl + 2) // 3) * 294 <= ((ntl + 1) // 2) * 232
     kname, fma_lanes = {F.FDD_KERNEL_SYMMETRIC2: ("k_rotate_sum_sym2<%d>" % (3 if ns3 else 2),
                                                   111 * 2 / 96.0 if ns3 else 79 * 2 / 64.0),
+                        F.FDD_KERNEL_MIXED: ("k_rotate_sum_sym2 + k_rotate_sum_generic (mixed)",
+                                             111 * 2 / 96.0),
                         F.FDD_KERNEL_SYMMETRIC: ("k_rotate_sum_sym", 47 * 2 / 32.0)}.get(
         kernel, ("k_rotate_sum_generic", 4.0))
     executed = 2.0 * fma_lanes * elements / (sum_ms * 1e-3) * 1e-12

@@ -66,9 +66,12 @@ enum fdd_kernel {
     FDD_KERNEL_AUTO = 0,       /* symmetric kernel where the DM grid allows it, else generic     */
     FDD_KERNEL_GENERIC = 1,    /* any delay table: one exactly range-reduced phasor per element  */
     FDD_KERNEL_SYMMETRIC = 2,  /* DM tiles in arithmetic progression: paired +-m rows */
-    FDD_KERNEL_SYMMETRIC2 = 3  /* same, up to three adjacent 32-DM tiles per CTA sharing one phasor
+    FDD_KERNEL_SYMMETRIC2 = 3, /* same, up to three adjacent 32-DM tiles per CTA sharing one phasor
                                   recurrence; the groups follow the uniform segments of the DM
                                   plan (a group ends where the DM step changes)                  */
+    FDD_KERNEL_MIXED = 4       /* SYMMETRIC2 for the 32-DM tiles that are arithmetic progressions,
+                                  GENERIC for the few that are not (a DM plan whose step changes
+                                  inside a tile)                                                */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */
@@ -118,9 +121,11 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
  * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
  * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
- * allows: SYMMETRIC2 (uniform and piecewise-uniform DM plans), else GENERIC.  A plan whose DM step
- * changes INSIDE a 32-DM tile is not piecewise-uniform in this sense and runs on the (about seven
- * times slower) generic kernel: make the segments of a DM plan multiples of 32 trial DMs. */
+ * allows: SYMMETRIC2 (uniform DM grids, and piecewise-uniform DM plans whose segments are multiples
+ * of 32 trial DMs), MIXED (piecewise-uniform plans with any segment lengths: only the tiles that
+ * contain a step change run on the about seven times slower generic kernel; at least half of the
+ * tiles must be progressions), else GENERIC.  FDD_KERNEL_MIXED may be asked for whenever at least
+ * one tile is a progression. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 
 /* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(HERE, "csrc", "libfdd_b200.so")
 
 FDD_MODE_TIME, FDD_MODE_FOURIER = 0, 1
 FDD_KERNEL_AUTO, FDD_KERNEL_GENERIC, FDD_KERNEL_SYMMETRIC, FDD_KERNEL_SYMMETRIC2 = 0, 1, 2, 3
+FDD_KERNEL_MIXED = 4
 FDD_OK = 0
 FDD_NUM_STAGES = 6
 STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift_add")

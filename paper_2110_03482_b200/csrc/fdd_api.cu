@@ -164,12 +164,16 @@ inline unsigned long long cycles_to_fixed64(long double cyc)
 int resolve_kernel(const fdd_plan* p, int request)
 {
     const bool sym2_ok = p->sym_ok;      // groups of sub-tiles follow the DM plan's uniform segments
+    const bool any_ap = p->sym.nap > 0;
     switch (request) {
         case FDD_KERNEL_GENERIC: return FDD_KERNEL_GENERIC;
         case FDD_KERNEL_SYMMETRIC: return p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC;
+        case FDD_KERNEL_MIXED: return sym2_ok ? FDD_KERNEL_SYMMETRIC2
+                                              : (any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC);
         default:
-            return sym2_ok ? FDD_KERNEL_SYMMETRIC2
-                           : (p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC);
+            if (sym2_ok) return FDD_KERNEL_SYMMETRIC2;
+            // a few tiles hold a change of DM step: those rows alone take the generic kernel
+            return 2 * p->sym.nap >= p->sym.ntiles && any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC;
     }
 }
 
@@ -408,15 +412,15 @@ int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
 // a4 on DM rows [j_begin, j_begin + rows) into dst (row pitch opitch float2).
 // mirror (SYMMETRIC2, TIME mode only): dst receives the pre-twiddled Z of the half-length inverse
 // transform instead of Y (fdd_kernels_sym2.cuh).
-int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
-                      cudaStream_t s, bool mirror = false)
+int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, float2* dst,
+                             long long opitch, int mode, cudaStream_t s, bool mirror)
 {
     const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
     const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
-    if (p->kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
+    if (kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
         // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of
         // one group per (channel, warp): 294 cycles for NS = 3, 232 for NS = 2
         const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
@@ -431,7 +435,7 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
                                       rows, dst, opitch, scale, real_edges, dc_add, s);
     }
     // (a chunk that does not start on a 32-DM tile - only with rows of > 0.75 GiB - goes generic)
-    if ((p->kernel == FDD_KERNEL_SYMMETRIC || p->kernel == FDD_KERNEL_SYMMETRIC2) &&
+    if ((kernel == FDD_KERNEL_SYMMETRIC || kernel == FDD_KERNEL_SYMMETRIC2) &&
         j_begin % fdd::kSymT == 0)
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);
@@ -442,6 +446,31 @@ int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long
         p->X, p->xpitch, p->phase64, p->ndm_pad, p->nchans, p->nbins_out, j_begin + rows, j_begin, n_jt,
         dst, opitch, scale, real_edges, dc_add);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
+// a4 with the plan's kernel; FDD_KERNEL_MIXED: runs of 32-DM tiles that are arithmetic progressions
+// take the shared-recurrence kernel, the tiles in between (a change of DM step inside them) the
+// generic one.
+int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
+                      cudaStream_t s, bool mirror = false)
+{
+    if (p->kernel != FDD_KERNEL_MIXED || j_begin % fdd::kSymT != 0)
+        return launch_rotate_sum_kernel(p, p->kernel == FDD_KERNEL_MIXED ? FDD_KERNEL_GENERIC : p->kernel,
+                                        j_begin, rows, dst, opitch, mode, s, mirror);
+    const int t0 = j_begin / fdd::kSymT, t1 = (j_begin + rows + fdd::kSymT - 1) / fdd::kSymT;
+    for (int t = t0; t < t1;) {
+        const bool ap = p->sym.ap[t] != 0;
+        int e = t + 1;
+        while (e < t1 && (p->sym.ap[e] != 0) == ap) ++e;
+        const int jb = t * fdd::kSymT;
+        const int je = e * fdd::kSymT < j_begin + rows ? e * fdd::kSymT : j_begin + rows;
+        const int rc = launch_rotate_sum_kernel(p, ap ? FDD_KERNEL_SYMMETRIC2 : FDD_KERNEL_GENERIC, jb,
+                                                je - jb, dst + (long long)(jb - j_begin) * opitch,
+                                                opitch, mode, s, false);
+        if (rc != FDD_OK) return rc;
+        t = e;
+    }
+    return FDD_OK;
 }
 
 int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst, cudaStream_t s,
@@ -653,7 +682,8 @@ int fdd_plan_get_output_shape(const fdd_plan* p, long long* nsamps_out, long lon
 int fdd_plan_set_kernel(fdd_plan* p, int kernel)
 {
     if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
-    if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_SYMMETRIC2) return FDD_ERR_INVALID_ARG;
+    if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_MIXED) return FDD_ERR_INVALID_ARG;
+    if (kernel == FDD_KERNEL_MIXED && p->sym.nap == 0) return FDD_ERR_UNSUPPORTED;
     if (kernel == FDD_KERNEL_SYMMETRIC && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     if (kernel == FDD_KERNEL_SYMMETRIC2 && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     p->kernel_request = kernel;

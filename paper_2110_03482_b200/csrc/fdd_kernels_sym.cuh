@@ -52,6 +52,11 @@ struct SymTables {
     // cont[t] != 0: sub-tile t + 1 continues the progression of sub-tile t (same half step, centre
     // 64 half steps on), so the two may share a CTA of fdd_kernels_sym2.cuh; host side only
     std::vector<unsigned char> cont;
+    // ap[t] != 0: sub-tile t is an arithmetic progression in every channel (host side only); a DM
+    // plan whose step changes inside a tile has a few tiles that are not, and those rows go to the
+    // generic kernel (FDD_KERNEL_MIXED)
+    std::vector<unsigned char> ap;
+    int nap = 0;            // number of such tiles
 };
 
 // For every adjacent pair of sub-tiles t, t+1: do they continue one arithmetic progression in every
@@ -85,6 +90,8 @@ inline void sym_free_tables(SymTables* t)
     t->bytes = 0;
     t->pair_ok = false;
     t->cont.clear();
+    t->ap.clear();
+    t->nap = 0;
 }
 
 inline unsigned long long sym_fixed64(long double cyc)
@@ -95,8 +102,9 @@ inline unsigned long long sym_fixed64(long double cyc)
     return (unsigned long long)(s + 0.5L);
 }
 
-// Build the per-tile tables; *ok = false (and no tables) if some tile is not an arithmetic
-// progression in every channel.  delays: host [ndm][nchans] in samples.
+// Build the per-tile tables; *ok = every tile is an arithmetic progression in every channel
+// (t->ap says which are; the table entries of the others are not used).  delays: host
+// [ndm][nchans] in samples.
 inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nchans, long long nfft,
                             bool* ok, size_t* scratch_bytes)
 {
@@ -105,6 +113,7 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
     *ok = false;
     const int ntiles = (ndm + kSymT - 1) / kSymT;
     std::vector<unsigned long long> hc((size_t)ntiles * nchans), hh((size_t)ntiles * nchans);
+    t->ap.assign(ntiles, 1);
     for (int tl = 0; tl < ntiles; ++tl) {
         const int j0 = tl * kSymT;
         const int r = ndm - j0 < kSymT ? ndm - j0 : kSymT;
@@ -118,7 +127,7 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
                 const long double want = d0 + step * i;
                 const long double got = delays[(size_t)(j0 + i) * nchans + c];
                 // 1e-8 samples is < 5e-9 cycles of phase at any bin
-                if (fabsl(got - want) > 1e-8L) return 0;
+                if (fabsl(got - want) > 1e-8L) t->ap[tl] = 0;
             }
             const long double h = step / 2;
             const long double dc = d0 + (kSymT - 1) * h;
@@ -140,11 +149,19 @@ inline int sym_build_tables(SymTables* t, const double* delays, int ndm, int nch
     }
     t->ntiles = ntiles;
     sym_continuations(hc, hh, ntiles, nchans, &t->cont);
+    t->nap = 0;
+    for (int tl = 0; tl < ntiles; ++tl) {
+        t->nap += t->ap[tl];
+        if (!t->ap[tl]) {                              // never grouped with a neighbour
+            t->cont[tl] = 0;
+            if (tl > 0) t->cont[tl - 1] = 0;
+        }
+    }
     t->pair_ok = true;
     for (int tl = 0; tl + 1 < ntiles; ++tl) t->pair_ok = t->pair_ok && t->cont[tl];
     t->bytes = 2 * bytes;
     if (scratch_bytes) *scratch_bytes += t->bytes;
-    *ok = true;
+    *ok = t->nap == ntiles;
     return 0;
 }
 

@@ -243,6 +243,35 @@ def test_kernel_selection_follows_the_dm_grid(F):
                     parity.assert_rows(_run(F, plan, u8, mode), ref, mode, "piecewise/32-DM tiles")
 
 
+def test_dm_plan_with_step_changes_inside_tiles_runs_mixed(F):
+    """A search-style DM plan (three ranges, each with its own step, lengths not multiples of 32):
+    AUTO = MIXED - the tiles that hold a step change take the generic kernel, the rest the
+    shared-recurrence one; against the fp64 oracle, both modes, and bit-compared with the generic
+    kernel on the rows of a generic tile."""
+    w = synth.small_workload(79, 40, 4096, 2)
+    u8 = synth.make_filterbank(w)
+    dms = np.concatenate([np.arange(50) * 0.5, 25.0 + np.arange(70) * 1.0, 95.0 + np.arange(45) * 2.0])
+    d = O.delay_table(40, w.f_lo, w.f_hi, w.tsamp, dms)
+    for mode in ("time", "fourier"):
+        ref = O.fdd_fft(u8, d, mode=mode)
+        with F.Plan.create(40, 4096, w.tsamp, w.f_lo, w.f_hi, dms) as plan:
+            assert plan.get_info()[5] == F.FDD_KERNEL_MIXED
+            with pytest.raises(F.FddError):
+                plan.set_kernel(F.FDD_KERNEL_SYMMETRIC2)
+            got = _run(F, plan, u8, mode)
+            parity.assert_rows(got, ref, mode, f"mixed/{mode}")
+            plan.set_kernel(F.FDD_KERNEL_GENERIC)
+            gen = _run(F, plan, u8, mode)
+            # trials 32..63 hold the first step change (at trial 50): generic in both runs
+            assert np.array_equal(got[32:64], gen[32:64])
+            assert not np.array_equal(got[0:32], gen[0:32])
+    rnd = np.sort(np.random.default_rng(8).uniform(0, 80, size=70))
+    with F.Plan.create(40, 4096, w.tsamp, w.f_lo, w.f_hi, rnd) as plan:
+        assert plan.get_info()[5] == F.FDD_KERNEL_GENERIC
+        with pytest.raises(F.FddError):
+            plan.set_kernel(F.FDD_KERNEL_MIXED)
+
+
 # ------------------------------------------------------------------ P3 on the GPU: exact integers
 def _integer_reference(u8, d, rows):
     ref = np.zeros((len(rows), u8.shape[0]), dtype=np.int64)
