@@ -11,7 +11,8 @@
  *                                          (Eq. 3; cuFFT)
  *   a4  phase-rotate-and-sum               Y[j][k] = sum_c X[c][k] e^{+2 pi i k d[j][c] / nfft}
  *                                          (Eq. 4 + Eq. 7; the hot kernel)
- *   a5  TIME:    batched complex-to-real FFT and 1/nfft scaling (Eq. 6)
+ *   a5  TIME:    batched inverse real FFT and 1/nfft scaling (Eq. 6; cuFFT: a
+ *                half-length complex transform of the pre-twiddled spectrum a4 writes, or C2R)
  *       FOURIER: nothing -- Y is the output (periodicity searches)
  *
  * with the delay table (a1, Eq. 1, against the highest channel)
@@ -31,7 +32,8 @@
  *     DEVICE memory of the current CUDA device.  The caller owns in_u8 and out; the plan owns
  *     every table, scratch buffer, cuFFT plan and workspace.  in_u8 is never modified.
  *   - A plan belongs to the device that was current at creation and is not re-entrant: at most
- *     one execute in flight per plan.  Different plans may run concurrently.
+ *     one execute in flight per plan.  Different plans may run concurrently.  Results are
+ *     deterministic: the same plan and input give the same bits on every execute.
  *   - Every function returns FDD_OK (0) or a negative fdd_status; nothing throws, nothing
  *     prints, no global state.  A failed create leaves *plan_out = NULL and frees everything.
  *   - There is no CPU fallback: without a CUDA device fdd_plan_create returns FDD_ERR_CUDA.
