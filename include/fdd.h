@@ -66,7 +66,8 @@ enum fdd_status {
 /* Kernel choice for step a4 (fdd_plan_set_kernel). */
 enum fdd_kernel {
     FDD_KERNEL_AUTO = 0,       /* symmetric kernel where the DM grid allows it, else generic     */
-    FDD_KERNEL_GENERIC = 1,    /* any delay table: one exactly range-reduced phasor per element  */
+    FDD_KERNEL_GENERIC = 1,    /* any delay table: phasors by recurrence along the bins from an
+                                  exactly range-reduced seed per (channel, DM, 8 bins)           */
     FDD_KERNEL_SYMMETRIC = 2,  /* DM tiles in arithmetic progression: paired +-m rows */
     FDD_KERNEL_SYMMETRIC2 = 3, /* same, up to three adjacent 32-DM tiles per CTA sharing one phasor
                                   recurrence; the groups follow the uniform segments of the DM
@@ -125,7 +126,7 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
  * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
  * allows: SYMMETRIC2 (uniform DM grids, and piecewise-uniform DM plans whose segments are multiples
  * of 32 trial DMs), MIXED (piecewise-uniform plans with any segment lengths: only the tiles that
- * contain a step change run on the about seven times slower generic kernel; at least half of the
+ * contain a step change run on the about 3.5 times slower generic kernel; at least half of the
  * tiles must be progressions), else GENERIC.  FDD_KERNEL_MIXED may be asked for whenever at least
  * one tile is a progression. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);

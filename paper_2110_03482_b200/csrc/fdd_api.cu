@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "fdd_kernels_generic.cuh"
+#include "fdd_kernels_krec.cuh"
 #include "fdd_kernels_pre.cuh"
 #include "fdd_kernels_sym.cuh"
 #include "fdd_kernels_sym2.cuh"
@@ -60,6 +61,11 @@ struct fdd_plan {
     long long ypitch = 0;
     int y_rows = 0;
     unsigned long long* phase64 = nullptr;   // generic kernel: [nchans][ndm_pad]
+    // bin-recurrence kernel (nfft <= 2^23): the same fractions as doubles * 2^(32 - pshift), and
+    // the per-bin phasor step exp(2 pi i frac(d / nfft)); [nchans][ndm_pad] each
+    double* rec_p32 = nullptr;
+    float2* rec_step = nullptr;
+    int rec_pshift = -1;                     // -1: series too long, generic kernel only
     int ndm_pad = 0;
     fdd::SymTables sym;                  // symmetric kernel tables (device) + tiling
     bool sym_ok = false;
@@ -186,6 +192,21 @@ int upload_generic_table(fdd_plan* p)
                 (long double)p->delays[(size_t)j * p->nchans + c] / (long double)p->nfft);
     if (cudaMemcpy(p->phase64, tab.data(), tab.size() * sizeof(unsigned long long),
                    cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_CUDA;
+    }
+    if (p->rec_pshift < 0) return FDD_OK;
+    // tables of the bin-recurrence kernel from the same 64-bit fractions
+    std::vector<double> p32(tab.size(), 0.0);
+    std::vector<float2> st(tab.size(), make_float2(1.f, 0.f));
+    const long double two_pi = 6.283185307179586476925286766559L;
+    for (size_t i = 0; i < tab.size(); ++i) {
+        const long double cyc = (long double)(long long)tab[i] * 5.42101086242752217e-20L;   // [-1/2, 1/2)
+        p32[i] = (double)ldexpl(cyc, 32 - p->rec_pshift);
+        st[i] = make_float2((float)cosl(two_pi * cyc), (float)sinl(two_pi * cyc));
+    }
+    if (cudaMemcpy(p->rec_p32, p32.data(), p32.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->rec_step, st.data(), st.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
@@ -319,6 +340,8 @@ void destroy_plan(fdd_plan* p)
     cudaFree(p->tdd_shifts);
     cudaFree(p->Y);
     cudaFree(p->phase64);
+    cudaFree(p->rec_p32);
+    cudaFree(p->rec_step);
     cudaFree(p->fft_ws);
     cudaFree(p->stage_in);
     cudaFree(p->stage_out);
@@ -349,6 +372,13 @@ int create_common(fdd_plan* p)
     if (rc != FDD_OK) return rc;
     rc = dev_alloc(p, &p->phase64, (size_t)p->nchans * p->ndm_pad);
     if (rc != FDD_OK) return rc;
+    p->rec_pshift = 0;
+    while ((p->nfft >> p->rec_pshift) > (1LL << 21)) ++p->rec_pshift;
+    if (p->rec_pshift > 2) p->rec_pshift = -1;           // > 2^23 points: integer phases only
+    if (p->rec_pshift >= 0) {
+        if ((rc = dev_alloc(p, &p->rec_p32, (size_t)p->nchans * p->ndm_pad)) != FDD_OK) return rc;
+        if ((rc = dev_alloc(p, &p->rec_step, (size_t)p->nchans * p->ndm_pad)) != FDD_OK) return rc;
+    }
     rc = build_tables(p);
     if (rc != FDD_OK) return rc;
     rc = make_fft_plans(p);
@@ -440,6 +470,16 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
         return fdd::sym_launch(p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin, rows,
                                dst, opitch, scale, real_edges, dc_add, s);
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
+    if (p->rec_pshift >= 0 && j_begin % fdd::kRecDT == 0) {
+        // any delay table, phasors by recurrence along the bins (fdd_kernels_krec.cuh)
+        const long long per_cta = (long long)fdd::kRecThreads * fdd::kRecL;
+        const long long n_kt = (p->nbins_out + per_cta - 1) / per_cta;
+        if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
+        fdd::k_rotate_sum_krec<<<(unsigned)(n_jt * n_kt), fdd::kRecThreads, 0, s>>>(
+            p->X, p->xpitch, p->rec_p32, p->rec_step, p->ndm_pad, p->nchans, p->nbins_out, j_begin + rows,
+            j_begin, n_jt, dst, opitch, scale, real_edges, dc_add, p->rec_pshift);
+        return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+    }
     const long long n_kt = (p->nbins_out + fdd::kGenThreads - 1) / fdd::kGenThreads;
     if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
     fdd::k_rotate_sum_generic<<<(unsigned)(n_jt * n_kt), fdd::kGenThreads, 0, s>>>(
