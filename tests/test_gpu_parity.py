@@ -147,10 +147,12 @@ def test_ragged_shapes(F, nchans, nsamps, ndm, step, dm0, mode, kernel):
         assert np.abs(got - ref).max() <= 1e-5 * scale
 
 
-@pytest.mark.parametrize("log2n,kernel", [(22, "symmetric"), (22, "auto"), (24, "auto")])
+@pytest.mark.parametrize("log2n,kernel", [(22, "symmetric"), (22, "auto"), (22, "generic"),
+                                          (24, "auto"), (24, "generic")])
 def test_long_series_phase_variants(F, oracle_c, log2n, kernel):
     """k_rotate_sum_sym2 forms its phases on the FP64 pipe with a reduced scale for
-    2^21 < nfft <= 2^23 and by integer multiplies beyond; k_rotate_sum_sym always by integers."""
+    2^21 < nfft <= 2^23 and by integer multiplies beyond; k_rotate_sum_sym always by integers;
+    FDD_KERNEL_GENERIC is the bin-recurrence kernel up to 2^23 points and the SFU kernel beyond."""
     w = synth.small_workload(321, 4, 1 << log2n, 70, dm_step=0.5, dm0=0.0)
     u8 = synth.make_filterbank(w)
     d = _delays_for(w)
