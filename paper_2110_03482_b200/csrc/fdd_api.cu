@@ -66,6 +66,7 @@ struct fdd_plan {
     double* rec_p32 = nullptr;
     float2* rec_step = nullptr;
     int rec_pshift = -1;                     // -1: series too long, generic kernel only
+    bool rec_ready = false;
     int ndm_pad = 0;
     fdd::SymTables sym;                  // symmetric kernel tables (device) + tiling
     bool sym_ok = false;
@@ -195,21 +196,39 @@ int upload_generic_table(fdd_plan* p)
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
-    if (p->rec_pshift < 0) return FDD_OK;
-    // tables of the bin-recurrence kernel from the same 64-bit fractions
-    std::vector<double> p32(tab.size(), 0.0);
-    std::vector<float2> st(tab.size(), make_float2(1.f, 0.f));
+    p->rec_ready = false;                // rebuilt on the next generic launch (ensure_rec_tables)
+    return FDD_OK;
+}
+
+// Tables of the bin-recurrence kernel, made on its first launch (plans on uniform DM grids never
+// need them): the same fractions frac(d / nfft) as doubles * 2^(32 - pshift), and exp(2 pi i frac).
+int ensure_rec_tables(fdd_plan* p)
+{
+    if (p->rec_ready) return FDD_OK;
+    const size_t n = (size_t)p->nchans * p->ndm_pad;
+    int rc;
+    if (!p->rec_p32 && (rc = dev_alloc(p, &p->rec_p32, n)) != FDD_OK) return rc;
+    if (!p->rec_step && (rc = dev_alloc(p, &p->rec_step, n)) != FDD_OK) return rc;
+    std::vector<double> p32(n, 0.0);
+    std::vector<float2> st(n, make_float2(1.f, 0.f));
     const long double two_pi = 6.283185307179586476925286766559L;
-    for (size_t i = 0; i < tab.size(); ++i) {
-        const long double cyc = (long double)(long long)tab[i] * 5.42101086242752217e-20L;   // [-1/2, 1/2)
-        p32[i] = (double)ldexpl(cyc, 32 - p->rec_pshift);
-        st[i] = make_float2((float)cosl(two_pi * cyc), (float)sinl(two_pi * cyc));
-    }
-    if (cudaMemcpy(p->rec_p32, p32.data(), p32.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(p->rec_step, st.data(), st.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+    for (int j = 0; j < p->ndm; ++j)
+        for (int c = 0; c < p->nchans; ++c) {
+            const unsigned long long f = cycles_to_fixed64(
+                (long double)p->delays[(size_t)j * p->nchans + c] / (long double)p->nfft);
+            const long double cyc = (long double)(long long)f * 5.42101086242752217e-20L;   // [-1/2, 1/2)
+            const size_t i = (size_t)c * p->ndm_pad + j;
+            p32[i] = (double)ldexpl(cyc, 32 - p->rec_pshift);
+            st[i] = make_float2((float)cosl(two_pi * cyc), (float)sinl(two_pi * cyc));
+        }
+    // (the stream may still be reading the old tables of a plan whose k_dm was changed)
+    if (cudaDeviceSynchronize() != cudaSuccess ||
+        cudaMemcpy(p->rec_p32, p32.data(), n * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->rec_step, st.data(), n * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
+    p->rec_ready = true;
     return FDD_OK;
 }
 
@@ -375,10 +394,6 @@ int create_common(fdd_plan* p)
     p->rec_pshift = 0;
     while ((p->nfft >> p->rec_pshift) > (1LL << 21)) ++p->rec_pshift;
     if (p->rec_pshift > 2) p->rec_pshift = -1;           // > 2^23 points: integer phases only
-    if (p->rec_pshift >= 0) {
-        if ((rc = dev_alloc(p, &p->rec_p32, (size_t)p->nchans * p->ndm_pad)) != FDD_OK) return rc;
-        if ((rc = dev_alloc(p, &p->rec_step, (size_t)p->nchans * p->ndm_pad)) != FDD_OK) return rc;
-    }
     rc = build_tables(p);
     if (rc != FDD_OK) return rc;
     rc = make_fft_plans(p);
@@ -472,6 +487,8 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
     if (p->rec_pshift >= 0 && j_begin % fdd::kRecDT == 0) {
         // any delay table, phasors by recurrence along the bins (fdd_kernels_krec.cuh)
+        const int rcs = ensure_rec_tables(p);
+        if (rcs != FDD_OK) return rcs;
         const long long per_cta = (long long)fdd::kRecThreads * fdd::kRecL;
         const long long n_kt = (p->nbins_out + per_cta - 1) / per_cta;
         if ((long long)n_jt * n_kt > 2147483647LL) return FDD_ERR_UNSUPPORTED;
