@@ -305,6 +305,17 @@ def fdd_rows(in_u8: np.ndarray, delays: np.ndarray, rows: Iterable[int], mode: s
         c1 = min(c0 + chan_block, nchans)
         X = np.fft.rfft(unpack(in_u8[:, c0:c1], n), axis=-1)
         phase_rotate_sum_c(X, d[:, c0:c1], n, out=Y, accumulate=True)
+    return rows_from_spectrum(Y, n, nsamps, mode, log2_factor)
+
+
+def rows_from_spectrum(Y: np.ndarray, nfft: int, nsamps: int, mode: str = "time",
+                       log2_factor: int = 0) -> np.ndarray:
+    """O5 + O6 of the at-scale tier: the output rows that belong to the sums Y[j][0..N/2] of O4.
+
+    The last step of ``fdd_rows``, callable on its own so that tests which need the TIME, FOURIER
+    and reduced-length (row f3) outputs of the same DM rows run O1..O4 once.
+    """
+    n = int(nfft)
     if log2_factor:
         if mode == "fourier":
             return Y[..., :(n >> log2_factor) // 2 + 1]

@@ -211,3 +211,19 @@ def integer_delay_table(seed: int, ndm: int, nchans: int, max_delay: int) -> np.
         tab[j] = np.minimum(np.rint(scale * shape) + (jitter if j else 0), max_delay)
     tab[0] = 0.0
     return tab
+
+
+def integer_progression_delay_table(ndm: int, nchans: int, max_step: int, dm0: int = 0) -> np.ndarray:
+    """float64 [ndm][nchans] of exact integer delays d[j][c] = (dm0 + j) * a_c (pin P3).
+
+    a_c = rint(max_step * (nu_c^-2 - nu_hi^-2) / (nu_lo^-2 - nu_hi^-2)) on a 1200-1500 MHz band: an
+    integer number of samples per trial, max_step in channel 0 and zero in the top channel, so every
+    channel's delays are an arithmetic progression over the trials -- a uniform "DM grid" whose
+    delays all happen to be whole samples.  The result then has an exact integer definition
+    (a circular shift-and-sum) AND the plan qualifies for the kernels that need progressions.
+    """
+    nu = np.linspace(1200.0, 1500.0, nchans) if nchans > 1 else np.array([1500.0])
+    shape = (nu ** -2 - 1500.0 ** -2) / (1200.0 ** -2 - 1500.0 ** -2)
+    a = np.rint(max_step * shape)
+    j = dm0 + np.arange(ndm, dtype=np.float64)
+    return j[:, None] * a[None, :]

@@ -52,14 +52,11 @@ KERNELS = ["generic", "symmetric", "auto"]
 
 
 def _set_kernel(F, plan, which):
-    """auto = the fastest kernel the delay table allows (SYMMETRIC2 on uniform DM grids)."""
-    if which == "symmetric":
-        try:
-            plan.set_kernel(F.FDD_KERNEL_SYMMETRIC)
-        except F.FddError:
-            pytest.skip("delay table is not an arithmetic progression per DM tile")
-        return
-    plan.set_kernel(F.FDD_KERNEL_GENERIC if which == "generic" else F.FDD_KERNEL_AUTO)
+    """auto = the fastest kernel the delay table allows (SYMMETRIC2 on uniform DM grids).
+    Returns the kernel the plan resolved to (enum fdd_kernel)."""
+    plan.set_kernel({"generic": F.FDD_KERNEL_GENERIC, "symmetric": F.FDD_KERNEL_SYMMETRIC,
+                     "symmetric2": F.FDD_KERNEL_SYMMETRIC2, "auto": F.FDD_KERNEL_AUTO}[which])
+    return plan.get_info()[5]
 
 
 # ------------------------------------------------------------------ stages a2 + a3
@@ -276,60 +273,82 @@ def test_dm_plan_with_step_changes_inside_tiles_runs_mixed(F):
 
 # ------------------------------------------------------------------ P3 on the GPU: exact integers
 def _integer_reference(u8, d, rows):
+    rows = list(rows)
     ref = np.zeros((len(rows), u8.shape[0]), dtype=np.int64)
-    for i, j in enumerate(rows):
-        for c in range(u8.shape[1]):
-            ref[i] += np.roll(u8[:, c].astype(np.int64), -int(d[j, c]))
+    for c in range(u8.shape[1]):
+        col = u8[:, c].astype(np.int64)
+        for i, j in enumerate(rows):
+            ref[i] += np.roll(col, -int(d[j, c]))
     return ref
 
 
-@pytest.mark.parametrize("kernel", KERNELS)
-def test_integer_delays_equal_circular_shift_and_sum(F, kernel):
-    nchans, nsamps, ndm = 128, 1 << 14, 40
+@pytest.mark.parametrize("table,kernel", [("jitter", "generic"), ("jitter", "auto"),
+                                          ("progression", "symmetric"), ("progression", "symmetric2"),
+                                          ("progression", "auto"), ("progression", "generic")])
+def test_integer_delays_equal_circular_shift_and_sum(F, table, kernel):
+    """Pin P3 through every a4 kernel: whole-sample delays make the result an exact circular
+    shift-and-sum, so the reference is integer arithmetic with no FFT in it ("the same
+    results as with time-domain dedispersion").  "jitter": delays with no structure (bin-recurrence
+    kernel); "progression": d[j][c] = j a_c with integer a_c, which the paired-row kernels take."""
+    nchans, nsamps, ndm = 128, 1 << 14, 100
     u8 = np.random.default_rng(9).integers(0, 256, (nsamps, nchans), dtype=np.uint8)
-    d = synth.integer_delay_table(11, ndm, nchans, 3000)
+    d = synth.integer_delay_table(11, ndm, nchans, 3000) if table == "jitter" else \
+        synth.integer_progression_delay_table(ndm, nchans, 30)
     ref = _integer_reference(u8, d, range(ndm))
     with F.Plan.create_from_delays(nchans, nsamps, d) as plan:
-        _set_kernel(F, plan, kernel)
+        used = _set_kernel(F, plan, kernel)
+        want = {"generic": F.FDD_KERNEL_GENERIC, "symmetric": F.FDD_KERNEL_SYMMETRIC,
+                "symmetric2": F.FDD_KERNEL_SYMMETRIC2,
+                "auto": F.FDD_KERNEL_GENERIC if table == "jitter" else F.FDD_KERNEL_SYMMETRIC2}[kernel]
+        assert used == want
         got = _run(F, plan, u8, "time")
-    # integer sums of 128 bytes (<= 32640): fp32 path must land within 0.02 of the integer
+        o = _run(F, plan, u8, "fourier")
+    # integer sums of 128 bytes (<= 32640): fp32 path must land within 0.05 of the integer
     assert np.abs(got - ref).max() <= 0.05
     assert np.array_equal(np.rint(got).astype(np.int64), ref)
     parity.assert_rows(got, ref.astype(np.float64), "time", "integer delays")
+    # FOURIER output = forward DFT of the integer rows (library rfft of exact integers)
+    parity.assert_rows(o, np.fft.rfft(ref.astype(np.float64), axis=-1), "fourier", "integer delays")
 
 
 # ------------------------------------------------------------------ host-buffer entry point
-def test_execute_host_matches_execute(F):
+def test_execute_host_against_the_oracle(F):
+    """fdd_execute_host (host buffers, pinned and pageable) against the fp64 oracle, and bit-equal
+    to fdd_execute on device buffers."""
     import torch
     w = synth.small_workload(31, 64, 8192, 48)
     u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
     with _plan_for(F, w) as plan:
-        dev = _run(F, plan, u8, "time")
         h_in = torch.from_numpy(u8).pin_memory()
-        h_out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32).pin_memory()
+        h_out = torch.full((plan.ndm, plan.nsamps), float("nan"), dtype=torch.float32).pin_memory()
         plan.execute_host(h_in, h_out, F.FDD_MODE_TIME)
-        assert np.array_equal(h_out.numpy(), dev)
-        h_outf = torch.empty((plan.ndm, plan.nbins, 2), dtype=torch.float32)      # pageable
+        parity.assert_rows(h_out.numpy(), O.fdd_fft(u8, d, mode="time"), "time", "execute_host/time")
+        h_outf = torch.full((plan.ndm, plan.nbins, 2), float("nan"), dtype=torch.float32)   # pageable
         plan.execute_host(u8, h_outf, F.FDD_MODE_FOURIER)
-        devf = _run(F, plan, u8, "fourier")
-        assert np.array_equal(h_outf.numpy()[..., 0] + 1j * h_outf.numpy()[..., 1], devf)
+        gotf = h_outf.numpy()[..., 0] + 1j * h_outf.numpy()[..., 1]
+        parity.assert_rows(gotf, O.fdd_fft(u8, d, mode="fourier"), "fourier", "execute_host/fourier")
+        assert np.array_equal(h_out.numpy(), _run(F, plan, u8, "time"))
+        assert np.array_equal(gotf, _run(F, plan, u8, "fourier"))
 
 
 def test_execute_host_output_ring_wraps(F):
-    """More DM chunks (384 rows each) than the 3 the device-side output ring holds."""
+    """More DM chunks (384 rows each) than the 3 the device-side output ring holds: every row
+    against the fp64 oracle, both modes."""
     import torch
     w = synth.small_workload(32, 16, 2048, 4 * 384 + 50, dm_step=0.05)
     u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
     with _plan_for(F, w) as plan:
         for mode, shape in (("time", (plan.ndm, plan.nsamps)), ("fourier", (plan.ndm, plan.nbins, 2))):
-            dev = _run(F, plan, u8, mode)
-            h_out = torch.zeros(shape, dtype=torch.float32).pin_memory()
+            h_out = torch.full(shape, float("nan"), dtype=torch.float32).pin_memory()
             plan.execute_host(u8, h_out, F.FDD_MODE_TIME if mode == "time" else F.FDD_MODE_FOURIER)
             got = h_out.numpy()
             if mode == "fourier":
                 got = got[..., 0] + 1j * got[..., 1]
-            # not bit-equal: the 50-row tail chunk takes 64-DM groups, the one-launch path 96-DM ones
-            assert np.abs(got - dev).max() <= 1e-5 * np.abs(dev).max()
+            parity.assert_rows(got, O.fdd_fft(u8, d, mode=mode), mode, f"execute_host ring/{mode}")
+            dev = _run(F, plan, u8, mode)
+            # (the 50-row tail chunk takes 64-DM groups, the one-launch path 96-DM ones)
             assert np.array_equal(got[:384], dev[:384])
 
 
@@ -389,31 +408,89 @@ def _sampled_rows(ndm, n, seed):
     return sorted(rows)
 
 
-@pytest.mark.slow
-@pytest.mark.parametrize("name,nrows", [("config2", 16), ("config3", 8), ("config4", 8)])
-def test_full_size_time_configs(F, oracle_c, name, nrows):
-    """config4 = the 4096-DM sweep point bench.py times (same plan, same kernel choice)."""
+class _FullSize:
+    """Inputs and oracle spectra of the full-size configs, made once per test session.
+
+    Configs 3 and 4 share one input (seed 1003) and one DM step, so trial j is the same DM at
+    every point of the config-4 sweep: the oracle's O1..O4 run once per distinct DM row and O5
+    (O.rows_from_spectrum) once per output wanted of it."""
+    u8 = {}
+    Y = {}                                   # (input name, trial index) -> oracle Y row (complex128)
+
+    @classmethod
+    def input(cls, name):
+        key = "config3" if name in ("config3", "config4", "sweep") else name
+        if key not in cls.u8:
+            cls.u8[key] = synth.make_filterbank(synth.workload(key))
+        return key, cls.u8[key]
+
+    @classmethod
+    def spectrum_rows(cls, name, w, rows):
+        key, u8 = cls.input(name)
+        todo = [j for j in rows if (key, j) not in cls.Y]
+        if todo:
+            Y = O.fdd_rows(u8, _delays_for(w), todo, mode="fourier")
+            for j, y in zip(todo, Y):
+                cls.Y[(key, j)] = y
+        return np.stack([cls.Y[(key, j)] for j in rows])
+
+
+def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0):
+    """One full-size TIME execute at `ndm` trial DMs; sampled rows against the oracle."""
     import torch
-    w = synth.workload(name)
-    u8 = synth.make_filterbank(w)
-    d = _delays_for(w)
-    rows = _sampled_rows(w.ndm, nrows, w.seed)
-    ref = O.fdd_rows(u8, d, rows, mode="time")
+    w = synth.workload(name, ndm=ndm)
+    _, u8 = _FullSize.input(name)
+    Y = _FullSize.spectrum_rows(name, w, rows)
+    ref = O.rows_from_spectrum(Y, O.next_pow2(w.nsamps), w.nsamps, "time", decimate)
     with _plan_for(F, w) as plan:
         assert plan.get_info()[2] == w.nsamps - (w.ndm - 1)
+        assert plan.get_info()[5] == kernel_want
+        if decimate:
+            plan.set_decimation(decimate)
+        ns_out, _ = plan.output_shape()
         d_in = torch.from_numpy(u8).cuda()
-        out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        out = torch.empty((plan.ndm, ns_out), dtype=torch.float32, device="cuda")
         plan.execute(d_in, out, F.FDD_MODE_TIME)
         torch.cuda.synchronize()
         got = out[rows].cpu().numpy()
-        # properties that hold at any size: DM 0 is the exact channel sum; DC invariance (P7)
-        y0 = out[0].cpu().numpy()
-        assert np.array_equal(np.rint(y0).astype(np.int64), u8.astype(np.int64).sum(axis=1))
-        total = float(u8.astype(np.int64).sum())
-        sums = out.double().sum(dim=1).cpu().numpy()
-        assert np.abs(sums - total).max() <= 2e-6 * total
-    worst = parity.assert_rows(got, ref, "time", name)
-    print(name, "rows", rows, worst)
+        if not decimate:
+            # properties that hold at any size: DM 0 is the exact channel sum; DC invariance (P7)
+            y0 = out[0].cpu().numpy()
+            assert np.array_equal(np.rint(y0).astype(np.int64), u8.astype(np.int64).sum(axis=1))
+            total = float(u8.astype(np.int64).sum())
+            sums = out.double().sum(dim=1).cpu().numpy()
+            assert np.abs(sums - total).max() <= 2e-6 * total
+    worst = parity.assert_rows(got, ref, "time", f"{name}/{ndm}/decimate {decimate}")
+    print(name, ndm, "decimate", decimate, "rows", rows, worst)
+    return worst
+
+
+@pytest.mark.slow
+def test_full_size_config2(F, oracle_c):
+    w = synth.workload("config2")
+    _full_size_point(F, "config2", w.ndm, _sampled_rows(w.ndm, 16, w.seed), F.FDD_KERNEL_SYMMETRIC2)
+
+
+# trials that the sweep points share (so the oracle computes each once) + every point's last row
+_SWEEP_POOL = [0, 37, 101, 300, 777, 1500, 3000]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("ndm", [128, 256, 512, 1024, 2048, 4096])
+def test_full_size_config4_dm_sweep(F, oracle_c, ndm):
+    """BASELINE.json configs[3]: every point of the DM-count sweep on the config-3 input, in the
+    plan bench.py times (1024 = config 3; 4096 = the default bench workload; 128 takes the 64-DM
+    group instance of the sym2 kernel, the others 96-DM groups with different tails)."""
+    rows = sorted({j for j in _SWEEP_POOL if j < ndm} | {ndm - 1, ndm // 2 + 15, ndm // 2 + 16})
+    _full_size_point(F, "config4", ndm, rows, F.FDD_KERNEL_SYMMETRIC2)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("m", [1, 2, 3])
+def test_full_size_config4_decimated(F, oracle_c, m):
+    """Row f3 at config-4 size (512 trial DMs): reduced-length inverse transform."""
+    rows = sorted({j for j in _SWEEP_POOL if j < 512} | {511, 271, 272})
+    _full_size_point(F, "config4", 512, rows, F.FDD_KERNEL_SYMMETRIC2, decimate=m)
 
 
 @pytest.mark.slow
@@ -448,38 +525,51 @@ def test_full_size_config5_fourier(F, oracle_c):
 
 
 @pytest.mark.slow
-def test_paper_series_length_zero_padded(F, oracle_c):
-    """The paper's series (4 687 500 samples of 64 us, zero padded to 2^23) in its band
-    (1181-1581 MHz, trial DMs 0, 2, 4, ...), 16 of the 1024 channels: padding, the scaled FP64
-    phases (nfft = 2^23) and the padded C2R path at full length."""
-    w = synth.small_workload(1006, 16, 4687500, 128, f_lo=1181.0, f_hi=1581.0, dm_step=2.0)
+def test_paper_workload_at_its_own_shape(F, oracle_c):
+    """bench.py --workload paper at the paper's shape: 1024 channels x 4 687 500
+    samples of 64 us zero padded to 2^23, band 1181-1581 MHz, trial DMs 0, 2, 4, ...  With padding
+    the mean of the u8 data is not a single bin, so it goes through both fp32 transforms."""
+    import torch
+    w = synth.workload("paper", ndm=128)
     u8 = synth.make_filterbank(w)
     d = _delays_for(w)
-    rows = [0, 1, 31, 32, 95, 96, 127]
+    rows = [0, 1, 31, 64, 96, 127]
     ref = O.fdd_rows(u8, d, rows, mode="time")
     with _plan_for(F, w) as plan:
         assert plan.nfft == 1 << 23 and plan.get_info()[5] == F.FDD_KERNEL_SYMMETRIC2
-        got = _run(F, plan, u8, "time")[rows]
-    parity.assert_rows(got, ref, "time", "paper series length")
-
-
-@pytest.mark.slow
-def test_full_size_integer_delays(F):
-    """P3 at 1024 channels x 2^20 samples: no FFT anywhere in the reference."""
-    import torch
-    nchans, nsamps, ndm = 1024, 1 << 20, 64
-    w = synth.workload("config3")
-    u8 = synth.make_filterbank(w)
-    d = synth.integer_delay_table(13, ndm, nchans, 1023)
-    rows = [0, 1, 17, 31, 32, 40, 62, 63]
-    ref = _integer_reference(u8, d, rows)
-    with F.Plan.create_from_delays(nchans, nsamps, d) as plan:
         d_in = torch.from_numpy(u8).cuda()
         out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
         plan.execute(d_in, out, F.FDD_MODE_TIME)
         torch.cuda.synchronize()
         got = out[rows].cpu().numpy()
-    parity.assert_rows(got, ref.astype(np.float64), "time", "integer delays, full size")
+    worst = parity.assert_rows(got, ref, "time", "paper workload, 1024 channels")
+    print("paper shape rows", rows, worst)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("table", ["jitter", "progression"])
+def test_full_size_integer_delays(F, table):
+    """P3 at 1024 channels x 2^20 samples: no FFT anywhere in the reference.  "progression"
+    (d[j][c] = j a_c, integer a_c) runs the hot kernel of the bench path, k_rotate_sum_sym2 with
+    96-DM groups and the mirrored epilogue; "jitter" the bin-recurrence kernel."""
+    import torch
+    nchans, nsamps = 1024, 1 << 20
+    _, u8 = _FullSize.input("config3")
+    if table == "jitter":
+        ndm, d, want = 64, synth.integer_delay_table(13, 64, nchans, 1023), F.FDD_KERNEL_GENERIC
+        rows = [0, 1, 17, 31, 32, 40, 62, 63]
+    else:
+        ndm, d, want = 192, synth.integer_progression_delay_table(192, nchans, 5), F.FDD_KERNEL_SYMMETRIC2
+        rows = [0, 1, 15, 16, 31, 32, 95, 96, 111, 112, 190, 191]
+    ref = _integer_reference(u8, d, rows)
+    with F.Plan.create_from_delays(nchans, nsamps, d) as plan:
+        assert plan.get_info()[5] == want
+        d_in = torch.from_numpy(u8).cuda()
+        out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute(d_in, out, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        got = out[rows].cpu().numpy()
+    parity.assert_rows(got, ref.astype(np.float64), "time", f"integer delays ({table}), full size")
     # sums of 1024 bytes reach 1.3e5 where the fp32 ulp is 1/64: the rounded value is the integer
     assert np.abs(got - ref).max() <= 0.25
     assert np.array_equal(np.rint(got).astype(np.int64), ref)

@@ -278,6 +278,13 @@ def test_p10_tiers_agree_on_tiny(oracle_c):
     assert np.abs(Yb - Y_naive[:, bins]).max() <= 1e-11 * np.abs(Y_naive).max()
     Y_rows = O.fdd_rows(u8, d, rows, mode="fourier")
     assert np.abs(Y_rows - Y_naive).max() <= 1e-11 * np.abs(Y_naive).max()
+    # rows_from_spectrum is fdd_rows' last step (O5): from the NAIVE sums it gives the naive rows,
+    # full rate and reduced length
+    n = O.next_pow2(w.nsamps)
+    assert np.abs(O.rows_from_spectrum(Y_naive, n, w.nsamps) - y_naive).max() <= 1e-11 * scale
+    y_red = O.naive_irdft_reduced(Y_naive, n, w.nsamps, 2)
+    assert np.abs(O.rows_from_spectrum(Y_naive, n, w.nsamps, "time", 2) - y_red).max() <= 1e-11 * scale
+    assert np.array_equal(O.rows_from_spectrum(Y_naive, n, w.nsamps, "fourier", 2), Y_naive[:, :n // 8 + 1])
 
 
 def test_c_matches_numpy(oracle_c):
