@@ -18,15 +18,20 @@ configuration BASELINE.json's target is quoted on, config 4 at 4096 trial DMs (1
              by a register-resident FFMA2 loop
   cpu_baseline  the CPU oracle as it stands, timed on the host cores on a bounded sample
 
-N > 1 (torchrun): weak scaling by trial-DM range -- every rank dedisperses the same input over
-its own block of ndm trial DMs (rank r: trials r*ndm .. (r+1)*ndm - 1); no data-path collective
-(DESIGN.md "Multi-GPU").  --impl reference times the oracle (rank 0 only).
+N > 1: weak scaling by trial-DM range -- every rank dedisperses the same input over its own
+block of ndm trial DMs (rank r: trials r*ndm .. (r+1)*ndm - 1); no data-path collective
+(DESIGN.md "Multi-GPU").  One process per GPU: under torchrun the ranks are already there; a
+plain `python bench.py --gpus N` starts them itself (torch.distributed.run on 127.0.0.1) and
+fails if fewer than N GPUs are visible.  --impl reference times the oracle (rank 0 only).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -180,6 +185,46 @@ def oracle_sample(w, u8, nrows: int, cfft: int = 256):
     return rate, what, O.num_threads(), time.time() - t_start
 
 
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def naive_tiny_sample():
+    """the NAIVE oracle (O(N^2) transforms, fdd_naive) end to end on the
+    whole Tiny config (64 channels x 8192 samples x 32 trial DMs), with one thread and with all the
+    threads numpy's BLAS takes on this box."""
+    import synth
+    from oracle import fdd_oracle as O
+    w = synth.workload("tiny")
+    u8 = synth.make_filterbank(w)
+    d = O.delay_table(w.nchans, w.f_lo, w.f_hi, w.tsamp, w.dm_list)
+    out = {"workload": "config 1 (tiny), all 32 trial DMs, naive O(N^2) DFTs", "unit": UNIT}
+    try:
+        from threadpoolctl import threadpool_limits
+    except Exception:
+        threadpool_limits = None
+    if threadpool_limits is not None:
+        with threadpool_limits(limits=1):
+            t0 = time.time()
+            O.fdd_naive(u8, d, mode="time")
+            t1 = time.time() - t0
+        out["single_thread_s"] = t1
+        out["single_thread_value"] = w.ndm * w.nsamps / t1
+    t0 = time.time()
+    O.fdd_naive(u8, d, mode="time")
+    ta = time.time() - t0
+    out["all_cores_s"] = ta
+    out["all_cores_value"] = w.ndm * w.nsamps / ta
+    out["host_cores"] = os.cpu_count()
+    return out
+
+
 def run_reference(args, rank: int, world: int):
     """--impl reference: the oracle timed on the host cores, rank 0 only."""
     if rank != 0:
@@ -204,11 +249,22 @@ def run_reference(args, rank: int, world: int):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(w, 1),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
-                         "sample": what},
+                         "sample": what, "host_cores": os.cpu_count(), "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def kernel_source_hash() -> str:
+    """sha256 (first 16 hex) over the CUDA sources: ties static profile numbers to a source state."""
+    import glob
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2110_03482_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 
 
 def workload_config(w, world: int):
@@ -293,7 +349,11 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     if flush is not None:                                  # the flush is not part of the path
         ms_total = sum(stage_ms.values())
     t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    per_rank_ms = [ms_total / args.steps]
     if world > 1:
+        allt = [torch.zeros_like(t) for _ in range(world)]
+        dist.all_gather(allt, t)
+        per_rank_ms = [float(x.item()) / args.steps for x in allt]
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
     units = float(w.ndm) * w.nsamps * world               # DM-trials x samples, all ranks
@@ -342,7 +402,33 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-        e2e = {"value": units / (float(t_e2e.item()) / args.e2e_steps), "unit": UNIT,
+        # the host link's own rate for pinned copies of this size class, measured here, so the
+        # reader can see how close e2e is to the link limit (its time is mostly the copy back)
+        pcie = None
+        if host_memory == "pinned":
+            nprobe = min(h_out.numel(), 1 << 28)                     # <= 1 GiB of floats
+            hv, dv = h_out.view(-1)[:nprobe], out.view(-1)[:nprobe]
+            ea, eb, ec = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            dv_keep = dv.clone()
+            hv.copy_(dv, non_blocking=True)                          # warm-up
+            torch.cuda.synchronize()
+            ea.record(stream)
+            hv.copy_(dv, non_blocking=True)
+            eb.record(stream)
+            dv.copy_(hv, non_blocking=True)
+            ec.record(stream)
+            torch.cuda.synchronize()
+            dv.copy_(dv_keep)
+            del dv_keep
+            d2h = nprobe * 4e-9 / (ea.elapsed_time(eb) * 1e-3)
+            h2d = nprobe * 4e-9 / (eb.elapsed_time(ec) * 1e-3)
+            t_step = float(t_e2e.item()) / args.e2e_steps
+            pcie = {"d2h_gbs_pinned_copy": d2h, "h2d_gbs_pinned_copy": h2d,
+                    "probe_bytes": nprobe * 4,
+                    "e2e_d2h_gbs": int(h_out.numel()) * 4e-9 / t_step,
+                    "e2e_time_over_copy_floor": t_step / (int(h_out.numel()) * 4e-9 / d2h
+                                                         + int(h_in.numel()) * 1e-9 / h2d)}
+        e2e = {"value": units / (float(t_e2e.item()) / args.e2e_steps), "unit": UNIT, "pcie": pcie,
                "h2d_bytes_per_step": int(h_in.numel()) * world,
                "d2h_bytes_per_step": int(h_out.numel()) * 4 * world,
                "steps": args.e2e_steps, "host_memory": host_memory,
@@ -356,40 +442,53 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         return
 
     # ---- roofline of the dominant kernel (a4) ---------------------------------------------
+    # achieved = the FP32 FMA work the kernel EXECUTES (2 flop per FMA lane) over its mean launch
+    # duration, against the FP32 FMA rate measured live on this GPU: a fraction of the pipe's peak,
+    # always <= 1.  The symmetric kernels execute fewer FMAs per (dm, channel, bin) element than the 8
+    # flop of one complex MAC (paired rows, shared three-term recurrence), so the rate at which they
+    # retire the rotate-then-MAC model's work is reported beside it, not as a fraction of peak.
     elements = float(w.ndm) * w.nchans * nbins
     sum_ms = stage_ms["rotate_sum"] / args.steps
-    achieved = FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12
-    traffic = None
+    ntl = (w.ndm + 31) // 32
+    ns3 = ((ntl + 2) // 3) * 294 <= ((ntl + 1) // 2) * 232          # the library's rule (sym2_shape)
+    kname, fma_lanes = {
+        F.FDD_KERNEL_SYMMETRIC2: ("k_rotate_sum_sym2<%d>" % (3 if ns3 else 2),
+                                  111 * 2 / 96.0 if ns3 else 79 * 2 / 64.0),
+        F.FDD_KERNEL_MIXED: ("k_rotate_sum_sym2 + k_rotate_sum_krec (mixed)", 111 * 2 / 96.0),
+        F.FDD_KERNEL_SYMMETRIC: ("k_rotate_sum_sym", 47 * 2 / 32.0),
+        # bin-recurrence kernel: 4 FMA for the MAC + 4 for the advance on 7 of 8 bins
+        F.FDD_KERNEL_GENERIC: ("k_rotate_sum_krec", 7.5) if nfft <= (1 << 23)
+        else ("k_rotate_sum_generic", 4.0)}[kernel]
+    executed = 2.0 * fma_lanes * elements / (sum_ms * 1e-3) * 1e-12
+    src_hash = kernel_source_hash()
+    traffic, traffic_src, traffic_hash = None, None, None
     tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")   # from the committed ncu summaries
     if os.path.exists(tpath) and not args.decimate:
         key = f"{w.name}/{w.ndm}/kernel{kernel}"
         for ln in open(tpath):
             f = ln.strip().split(",")
-            if len(f) >= 2 and f[0] == key:
-                traffic = float(f[1])
-    # FMA lanes the kernel actually executes per element (accumulate + phasor recurrence):
-    # sym2 111 FFMA2 per 96 DMs (NS = 3) or 79 per 64 (NS = 2, the library's choice when that
-    # leaves fewer 32-DM sub-tiles idle), sym 47 FFMA2 per 32 DMs, generic 4 FFMA per element
-    ntl = (w.ndm + 31) // 32
-    ns3 = ((ntl + 2) // 3) * 294 <= ((ntl + 1) // 2) * 232
-    kname, fma_lanes = {F.FDD_KERNEL_SYMMETRIC2: ("k_rotate_sum_sym2<%d>" % (3 if ns3 else 2),
-                                                  111 * 2 / 96.0 if ns3 else 79 * 2 / 64.0),
-                        F.FDD_KERNEL_MIXED: ("k_rotate_sum_sym2 + k_rotate_sum_generic (mixed)",
-                                             111 * 2 / 96.0),
-                        F.FDD_KERNEL_SYMMETRIC: ("k_rotate_sum_sym", 47 * 2 / 32.0)}.get(
-        kernel, ("k_rotate_sum_generic", 4.0))
-    executed = 2.0 * fma_lanes * elements / (sum_ms * 1e-3) * 1e-12
+            if len(f) >= 3 and f[0] == key:
+                traffic, traffic_src = float(f[1]), f[2]
+                traffic_hash = f[3] if len(f) > 3 else None
     roofline = {
         "kernel": kname,
-        "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
-        "frac": achieved / peak_tf, "traffic": traffic,
+        "bound": "alu", "achieved": executed, "peak": peak_tf, "unit": "TFLOP/s",
+        "frac": executed / peak_tf, "traffic": traffic,
+        "traffic_source": None if traffic is None else
+        f"static: profiles/{traffic_src} (one ncu --set full capture, not this run)",
+        "traffic_stale": None if traffic is None else (traffic_hash != src_hash),
+        "kernel_sources_sha": src_hash,
         "peak_source": "measured live: fdd_measure_fp32_peak (FFMA2 register loop, all SMs, "
                        f"{peak_ms:.0f} ms); cross-check 148 SM x 128 lanes x 2 x 1.965 GHz = 74.45",
-        "algorithmic": "8 flop (one complex MAC) per (dm, channel, bin) element - the work of a "
-                       "rotate-then-MAC kernel without its phasor; the symmetric kernels execute "
-                       "fewer (paired rows + shared three-term recurrence), so frac can pass 1",
+        "achieved_is": "executed FP32 FMA lanes x 2 flop / mean launch duration (CUDA events "
+                       "around the stage, inside the timed region)",
         "executed_fma_lanes_per_element": fma_lanes,
-        "executed_tflops": executed, "executed_frac": executed / peak_tf,
+        "executed_fma_lanes_source": "static: FFMA2 counted in the SASS of the channel loop "
+                                     "(profiles/*_ncu_full_*.md instruction mix), not a counter of this run",
+        "algorithmic_equiv_tflops": FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12,
+        "algorithmic_equiv_is": "8 flop (one complex MAC) per (dm, channel, bin) element / time: the "
+                                "rate at which a rotate-then-MAC kernel would have to run to match; "
+                                "not a fraction of peak (this kernel executes fewer flop per element)",
         "ms_per_launch": sum_ms, "share_of_step": sum_ms / ms_step,
     }
     line = {
@@ -397,6 +496,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": dict(workload_config(w, world), decimation_log2=args.decimate),
+        "ms_per_step_per_rank": per_rank_ms,
         "tdd_comparator": tdd,
         "clocks": sampler.summary(),
         "e2e": e2e,
@@ -434,7 +534,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         torch.cuda.empty_cache()
         rate, what, threads, _ = oracle_sample(w, u8, args.cpu_rows)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": what, "host_cores": os.cpu_count()}
+                                "sample": what, "host_cores": os.cpu_count(),
+                                "cpu_model": cpu_model(), "naive_tiny": naive_tiny_sample()}
     else:
         plan.destroy()
     print(json.dumps(line), flush=True)
@@ -450,6 +551,19 @@ def main():
         return
     if world != args.gpus and world > 1:
         raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.gpus > 1 and world == 1:
+        # not under torchrun: start one process per GPU ourselves (same launch the driver uses)
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"--gpus {args.gpus} but only {have} CUDA device(s) are visible")
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+               f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     run_b200(args, rank, local_rank, world)
 
 

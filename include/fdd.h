@@ -3,7 +3,9 @@
  * Method: Bassa, Romein, Veenboer, van der Vlugt & Wijnholds, "Fourier-domain dedispersion",
  * arXiv:2110.03482.  Citations "PAPER.md:<line>" refer to the paper text the build was given.
  *
- * One fdd_execute() call runs, on one GPU and one CUDA stream, with no host synchronisation:
+ * One fdd_execute() call runs, on one GPU and one CUDA stream, with no host synchronisation once
+ * the plan has been prepared for that mode (fdd_plan_prepare; an unprepared plan does the same
+ * allocations inside its first execute, which may then synchronise the device):
  *
  *   a2  unpack + transpose (+ zero pad)   u8 [nsamps][nchans] -> f32 [nchans][nfft]
  *                                          (Algorithm 1 lines 10-11)
@@ -130,6 +132,28 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
  * tiles must be progressions), else GENERIC.  FDD_KERNEL_MIXED may be asked for whenever at least
  * one tile is a progression. */
 int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
+
+/* Make everything an fdd_execute / fdd_rotate_sum_only in `mode` (enum fdd_mode) needs that the plan
+ * creates lazily, so that the execute itself allocates nothing, uploads nothing and never
+ * synchronises (it can then be captured in a CUDA graph):
+ *   TIME     the Y scratch (up to 24 GiB, see fdd_plan_set_y_budget), the inverse cuFFT plans and
+ *            the shared cuFFT workspace
+ *   both     the bin-recurrence tables if any trial DM runs on FDD_KERNEL_GENERIC, and the launch
+ *            shapes (DM-tile groups) of the shared-recurrence kernel
+ * Call it again after fdd_plan_set_kernel, fdd_plan_set_kdm, fdd_plan_set_decimation or
+ * fdd_plan_set_y_budget.  Synchronises the device.  Not needed for correctness: an unprepared plan
+ * does the same work inside its first execute.  (The staging buffers of fdd_execute_host and the
+ * tables of fdd_tdd_execute are still made on their first call.) */
+int fdd_plan_prepare(fdd_plan *plan, int mode);
+
+/* TIME mode keeps the sums Y of a chunk of trial DMs in plan-owned scratch between a4 and a5.  The
+ * chunk is as many rows as fit `bytes` (default 24 GiB, and never more than half of the free
+ * device memory), rounded down to whole inverse-FFT batches (384 rows), 96-DM groups, 32-DM tiles
+ * or multiples of 8 rows; plans with more trial DMs run a4 + a5 chunk after chunk (the paper's
+ * DM_outer batches, without re-doing a2 + a3).  bytes = 0 restores the default.
+ * FDD_ERR_ALLOC from the next TIME execute / prepare if not even 8 rows fit.  Synchronises the
+ * device and drops the TIME-mode scratch. */
+int fdd_plan_set_y_budget(fdd_plan *plan, size_t bytes);
 
 /* Run a2..a5 asynchronously on cuda_stream (a cudaStream_t passed as void*; NULL = legacy
  * default stream).

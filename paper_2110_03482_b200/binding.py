@@ -22,7 +22,8 @@ STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift
 
 EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
-    "fdd_plan_set_decimation", "fdd_plan_get_output_shape",
+    "fdd_plan_set_decimation", "fdd_plan_get_output_shape", "fdd_plan_prepare",
+    "fdd_plan_set_y_budget",
     "fdd_execute", "fdd_execute_host", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_error_string",
@@ -63,6 +64,8 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_get_delays.argtypes = [vp, P(c_dbl)]
     lib.fdd_plan_set_profiling.argtypes = [vp, c_int]
     lib.fdd_plan_set_decimation.argtypes = [vp, c_int]
+    lib.fdd_plan_prepare.argtypes = [vp, c_int]
+    lib.fdd_plan_set_y_budget.argtypes = [vp, ctypes.c_size_t]
     lib.fdd_plan_get_output_shape.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong),
                                               ctypes.POINTER(ctypes.c_longlong)]
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
@@ -190,6 +193,14 @@ class Plan:
         """Reduced-length inverse transform = down-sampling by 2^log2_factor."""
         _check(load_library().fdd_plan_set_decimation(self._h, int(log2_factor)),
                "fdd_plan_set_decimation")
+
+    def prepare(self, mode: int = FDD_MODE_TIME) -> None:
+        """Do every lazy allocation / upload of ``mode`` now, so execute never synchronises."""
+        _check(load_library().fdd_plan_prepare(self._h, int(mode)), "fdd_plan_prepare")
+
+    def set_y_budget(self, nbytes: int) -> None:
+        """Cap the TIME-mode Y scratch (trial DMs are then processed in chunks); 0 = default."""
+        _check(load_library().fdd_plan_set_y_budget(self._h, int(nbytes)), "fdd_plan_set_y_budget")
 
     def output_shape(self) -> Tuple[int, int]:
         """(floats per TIME row, float2 per FOURIER row) after set_decimation."""

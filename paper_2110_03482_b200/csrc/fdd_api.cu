@@ -9,7 +9,9 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <map>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "fdd_kernels_generic.cuh"
@@ -67,7 +69,12 @@ struct fdd_plan {
     float2* rec_step = nullptr;
     int rec_pshift = -1;                     // -1: series too long, generic kernel only
     bool rec_ready = false;
+    std::vector<double> rec_p32_host;        // plan-owned upload buffers (asynchronous copies read them)
+    std::vector<float2> rec_step_host;
     int ndm_pad = 0;
+    size_t y_budget = 0;                     // TIME-mode Y scratch budget in bytes (fdd_plan_set_y_budget)
+    // a4 launch shapes of the shared-recurrence kernel, made once per (first row, rows) chunk
+    std::map<std::pair<int, int>, fdd::Sym2Shape> sym2_shapes;
     fdd::SymTables sym;                  // symmetric kernel tables (device) + tiling
     bool sym_ok = false;
     int kernel = FDD_KERNEL_GENERIC;     // resolved choice
@@ -156,15 +163,7 @@ void finish_delay_stats(fdd_plan* p)
     p->max_delay = m;
     // S10: mathematically integer delays may evaluate a hair above the integer
     p->valid_len = p->nsamps - (long long)ceil(m * (1.0 - 1e-12));
-}
-
-// frac(d / nfft) as a 64-bit binary fraction of a cycle.
-inline unsigned long long cycles_to_fixed64(long double cyc)
-{
-    long double f = cyc - floorl(cyc);                   // [0, 1)
-    long double s = f * 18446744073709551616.0L;         // * 2^64
-    if (s >= 18446744073709551615.0L) return 0ULL;       // rounds up to a whole cycle
-    return (unsigned long long)(s + 0.5L);
+    if (p->valid_len < 0) p->valid_len = 0;          // delays longer than the series: nothing is valid
 }
 
 // AUTO: the fastest kernel the delay table allows.
@@ -189,42 +188,51 @@ int upload_generic_table(fdd_plan* p)
     std::vector<unsigned long long> tab((size_t)p->nchans * p->ndm_pad, 0ULL);
     for (int j = 0; j < p->ndm; ++j)
         for (int c = 0; c < p->nchans; ++c)
-            tab[(size_t)c * p->ndm_pad + j] = cycles_to_fixed64(
+            tab[(size_t)c * p->ndm_pad + j] = fdd::sym_fixed64(
                 (long double)p->delays[(size_t)j * p->nchans + c] / (long double)p->nfft);
+    // (a cudaMemcpy from pageable memory returns once the data are staged; the synchronize makes
+    // sure they have landed before a kernel on a non-blocking stream can read them)
     if (cudaMemcpy(p->phase64, tab.data(), tab.size() * sizeof(unsigned long long),
-                   cudaMemcpyHostToDevice) != cudaSuccess) {
+                   cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaDeviceSynchronize() != cudaSuccess) {
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
-    p->rec_ready = false;                // rebuilt on the next generic launch (ensure_rec_tables)
+    p->rec_ready = false;                // rebuilt by fdd_plan_prepare / the next generic launch
+    p->sym2_shapes.clear();
     return FDD_OK;
 }
 
-// Tables of the bin-recurrence kernel, made on its first launch (plans on uniform DM grids never
-// need them): the same fractions frac(d / nfft) as doubles * 2^(32 - pshift), and exp(2 pi i frac).
-int ensure_rec_tables(fdd_plan* p)
+// Tables of the bin-recurrence kernel (plans on uniform DM grids never need them): the same
+// fractions frac(d / nfft) as doubles * 2^(32 - pshift), and exp(2 pi i frac).  Made by
+// fdd_plan_prepare, or by the first generic launch of a plan that was not prepared: then the
+// device buffers are allocated here (cudaMalloc may synchronise) and the upload is queued on the
+// launching stream from plan-owned host buffers, in order with the kernel that reads them.
+int ensure_rec_tables(fdd_plan* p, cudaStream_t s)
 {
     if (p->rec_ready) return FDD_OK;
     const size_t n = (size_t)p->nchans * p->ndm_pad;
     int rc;
     if (!p->rec_p32 && (rc = dev_alloc(p, &p->rec_p32, n)) != FDD_OK) return rc;
     if (!p->rec_step && (rc = dev_alloc(p, &p->rec_step, n)) != FDD_OK) return rc;
-    std::vector<double> p32(n, 0.0);
-    std::vector<float2> st(n, make_float2(1.f, 0.f));
+    // (the host buffers may still feed an earlier upload of a plan whose k_dm was changed)
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return FDD_ERR_CUDA; }
+    p->rec_p32_host.assign(n, 0.0);
+    p->rec_step_host.assign(n, make_float2(1.f, 0.f));
     const long double two_pi = 6.283185307179586476925286766559L;
     for (int j = 0; j < p->ndm; ++j)
         for (int c = 0; c < p->nchans; ++c) {
-            const unsigned long long f = cycles_to_fixed64(
+            const unsigned long long f = fdd::sym_fixed64(
                 (long double)p->delays[(size_t)j * p->nchans + c] / (long double)p->nfft);
             const long double cyc = (long double)(long long)f * 5.42101086242752217e-20L;   // [-1/2, 1/2)
             const size_t i = (size_t)c * p->ndm_pad + j;
-            p32[i] = (double)ldexpl(cyc, 32 - p->rec_pshift);
-            st[i] = make_float2((float)cosl(two_pi * cyc), (float)sinl(two_pi * cyc));
+            p->rec_p32_host[i] = (double)ldexpl(cyc, 32 - p->rec_pshift);
+            p->rec_step_host[i] = make_float2((float)cosl(two_pi * cyc), (float)sinl(two_pi * cyc));
         }
-    // (the stream may still be reading the old tables of a plan whose k_dm was changed)
-    if (cudaDeviceSynchronize() != cudaSuccess ||
-        cudaMemcpy(p->rec_p32, p32.data(), n * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(p->rec_step, st.data(), n * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+    if (cudaMemcpyAsync(p->rec_p32, p->rec_p32_host.data(), n * sizeof(double), cudaMemcpyHostToDevice,
+                        s) != cudaSuccess ||
+        cudaMemcpyAsync(p->rec_step, p->rec_step_host.data(), n * sizeof(float2),
+                        cudaMemcpyHostToDevice, s) != cudaSuccess) {
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
@@ -286,23 +294,38 @@ int make_c2r_plan(fdd_plan* p, int family, cufftHandle* h, int batch, size_t* ws
     return FDD_OK;
 }
 
-// TIME-mode resources are allocated on the first TIME execute (a FOURIER-only plan such as
-// config 5 never needs the 16 GiB of Y).
-int ensure_time_resources(fdd_plan* p, int family = 0)
+// The a5 family the plan's kernel feeds: 1 = the half-length complex inverse of the pre-twiddled
+// spectrum the mirrored sym2 epilogue writes, 0 = cuFFT's C2R from Y.
+int time_family(const fdd_plan* p)
+{
+    return (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
+}
+
+void drop_c2r_plan(cufftHandle* h, bool* have)
+{
+    if (*have) cufftDestroy(*h);
+    *have = false;
+}
+
+// TIME-mode resources (a FOURIER-only plan such as config 5 never needs the 16 GiB of Y): made by
+// fdd_plan_prepare(TIME), or by the first TIME execute of a plan that was not prepared.
+int ensure_time_resources(fdd_plan* p, int family)
 {
     int rc;
     if (!p->Y) {
         p->ypitch = round_up(p->nbins_out, kPitchAlign);
         const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
-        long long rows = (long long)(kYBudgetBytes / row_bytes);
+        long long rows = (long long)((p->y_budget ? p->y_budget : kYBudgetBytes) / row_bytes);
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
             long long fit = (long long)(free_b / 2 / row_bytes);
             if (fit < rows) rows = fit;
         }
+        // DM chunks: whole cuFFT batches (4 x 96-DM groups) if possible, else whole 96-DM groups,
+        // else whole 32-DM tiles, else multiples of 8 (the generic kernels' DM tile)
         if (rows >= p->ndm) rows = p->ndm;
-        else rows = rows >= kC2RBatch ? rows / kC2RBatch * kC2RBatch          // whole 96-DM groups
-                                      : (rows >= 96 ? rows / 96 * 96 : (rows >= 32 ? 32 : rows));
+        else rows = rows >= kC2RBatch ? rows / kC2RBatch * kC2RBatch
+                                      : (rows >= 96 ? rows / 96 * 96 : (rows >= 32 ? 32 : rows / 8 * 8));
         if (rows < 1) return FDD_ERR_ALLOC;
         p->y_rows = (int)rows;
         p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
@@ -316,30 +339,65 @@ int ensure_time_resources(fdd_plan* p, int family = 0)
     if (p->have_c2r[family]) return FDD_OK;
     size_t ws_a = 0, ws_b = 0;
     rc = make_c2r_plan(p, family, &p->c2r[family], p->c2r_batch, &ws_a);
-    p->have_c2r[family] = true;
-    if (rc != FDD_OK) return rc;
-    if (p->c2r_tail_batch) {
+    p->have_c2r[family] = true;                  // (the handle exists; dropped below on failure)
+    if (rc == FDD_OK && p->c2r_tail_batch) {
         rc = make_c2r_plan(p, family, &p->c2r_tail[family], p->c2r_tail_batch, &ws_b);
         p->have_c2r_tail[family] = true;
-        if (rc != FDD_OK) return rc;
     }
     const size_t need = ws_a > ws_b ? ws_a : ws_b;
-    if (need > p->fft_ws_bytes) {
+    if (rc == FDD_OK && need > p->fft_ws_bytes) {
         // (no execute is in flight on a plan that is being grown: plans are not re-entrant)
-        if (cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
-        if (p->fft_ws) { cudaFree(p->fft_ws); p->scratch_bytes -= p->fft_ws_bytes; p->fft_ws = nullptr; }
-        p->fft_ws_bytes = 0;
-        rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->fft_ws), need);
-        if (rc != FDD_OK) return rc;
-        p->fft_ws_bytes = need;
+        if (cudaDeviceSynchronize() != cudaSuccess) rc = FDD_ERR_CUDA;
+        if (rc == FDD_OK) {
+            if (p->fft_ws) { cudaFree(p->fft_ws); p->scratch_bytes -= p->fft_ws_bytes; p->fft_ws = nullptr; }
+            p->fft_ws_bytes = 0;
+            rc = dev_alloc(p, reinterpret_cast<unsigned char**>(&p->fft_ws), need);
+            if (rc == FDD_OK) p->fft_ws_bytes = need;
+        }
     }
     // every plan works in the one shared area (never two transforms in flight)
-    if (cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    for (int f = 0; f < 2; ++f) {
-        if (p->have_c2r[f] && cufftSetWorkArea(p->c2r[f], p->fft_ws) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    if (rc == FDD_OK && cufftSetWorkArea(p->r2c, p->fft_ws) != CUFFT_SUCCESS) rc = FDD_ERR_CUFFT;
+    for (int f = 0; f < 2 && rc == FDD_OK; ++f) {
+        if (p->have_c2r[f] && cufftSetWorkArea(p->c2r[f], p->fft_ws) != CUFFT_SUCCESS) rc = FDD_ERR_CUFFT;
         if (p->have_c2r_tail[f] && cufftSetWorkArea(p->c2r_tail[f], p->fft_ws) != CUFFT_SUCCESS)
-            return FDD_ERR_CUFFT;
+            rc = FDD_ERR_CUFFT;
     }
+    if (rc != FDD_OK) {
+        // a half-made handle must not survive: the next execute starts this family from scratch
+        drop_c2r_plan(&p->c2r[family], &p->have_c2r[family]);
+        drop_c2r_plan(&p->c2r_tail[family], &p->have_c2r_tail[family]);
+    }
+    return rc;
+}
+
+void drop_time_resources(fdd_plan* p)
+{
+    for (int f = 0; f < 2; ++f) {
+        drop_c2r_plan(&p->c2r[f], &p->have_c2r[f]);
+        drop_c2r_plan(&p->c2r_tail[f], &p->have_c2r_tail[f]);
+    }
+    if (p->Y) {
+        cudaFree(p->Y);
+        p->scratch_bytes -= (size_t)p->y_rows * p->ypitch * sizeof(float2);
+        p->Y = nullptr;
+    }
+    p->y_rows = 0;
+    p->c2r_tail_batch = 0;
+    p->sym2_shapes.clear();
+}
+
+// Both TIME-mode families a chunked run may need (a Y chunk off the 32-DM tiling falls back to
+// cuFFT's C2R); returns the family to use.
+int ensure_time_family(fdd_plan* p, int* family_out)
+{
+    int family = time_family(p);
+    int rc = ensure_time_resources(p, family);
+    if (rc != FDD_OK) return rc;
+    if (family == 1 && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0) {
+        family = 0;                          // chunks off the 32-DM tiling run the generic kernel
+        if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
+    }
+    *family_out = family;
     return FDD_OK;
 }
 
@@ -466,18 +524,17 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
     if (kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
-        // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of
-        // one group per (channel, warp): 294 cycles for NS = 3, 232 for NS = 2
-        const int ntl = (rows + fdd::kSymT - 1) / fdd::kSymT;
-        std::vector<unsigned short> gs;
-        std::vector<unsigned char> gc;
-        const long long cost3 = 294LL * fdd::sym2_group(p->sym, j_begin / fdd::kSymT, ntl, 3, &gs, &gc);
-        const long long cost2 = 232LL * fdd::sym2_group(p->sym, j_begin / fdd::kSymT, ntl, 2, &gs, &gc);
-        if (cost3 <= cost2)
-            return fdd::sym2_launch<3, 2>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
-                                          rows, dst, opitch, scale, real_edges, dc_add, s);
-        return fdd::sym2_launch<2, 3>(mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm, j_begin,
-                                      rows, dst, opitch, scale, real_edges, dc_add, s);
+        // the grouping of the chunk's 32-DM sub-tiles is made once per (first row, rows)
+        auto it = p->sym2_shapes.find(std::make_pair(j_begin, rows));
+        if (it == p->sym2_shapes.end())
+            it = p->sym2_shapes.emplace(std::make_pair(j_begin, rows),
+                                        fdd::sym2_shape(p->sym, j_begin, rows)).first;
+        const fdd::Sym2Shape& sh = it->second;
+        if (sh.ns == 3)
+            return fdd::sym2_launch<3, 2>(sh, mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out,
+                                          p->ndm, j_begin, rows, dst, opitch, scale, real_edges, dc_add, s);
+        return fdd::sym2_launch<2, 3>(sh, mirror, p->nfft, p->sym, p->X, p->xpitch, p->nchans, p->nbins_out,
+                                      p->ndm, j_begin, rows, dst, opitch, scale, real_edges, dc_add, s);
     }
     // (a chunk that does not start on a 32-DM tile - only with rows of > 0.75 GiB - goes generic)
     if ((kernel == FDD_KERNEL_SYMMETRIC || kernel == FDD_KERNEL_SYMMETRIC2) &&
@@ -487,7 +544,7 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     const int n_jt = (rows + fdd::kGenDT - 1) / fdd::kGenDT;
     if (p->rec_pshift >= 0 && j_begin % fdd::kRecDT == 0) {
         // any delay table, phasors by recurrence along the bins (fdd_kernels_krec.cuh)
-        const int rcs = ensure_rec_tables(p);
+        const int rcs = ensure_rec_tables(p, s);
         if (rcs != FDD_OK) return rcs;
         const long long per_cta = (long long)fdd::kRecThreads * fdd::kRecL;
         const long long n_kt = (p->nbins_out + per_cta - 1) / per_cta;
@@ -610,13 +667,9 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         return FDD_OK;
     }
     // SYMMETRIC2 writes the pre-twiddled spectrum of the half-length complex inverse (family 1)
-    int family = (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
-    int rc = ensure_time_resources(p, family);
+    int family = 0;
+    int rc = ensure_time_family(p, &family);
     if (rc != FDD_OK) return rc;
-    if (family == 1 && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0) {
-        family = 0;                          // chunks off the 32-DM tiling run the generic kernel
-        if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
-    }
     const int step = (chunk_rows > 0 && chunk_rows < p->y_rows) ? chunk_rows : p->y_rows;
     for (int j0 = 0; j0 < p->ndm; j0 += step) {
         const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
@@ -710,17 +763,9 @@ int fdd_plan_set_decimation(fdd_plan* p, int log2_factor)
         return FDD_ERR_INVALID_ARG;
     DeviceGuard g(p->device);
     if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
-    // the TIME-mode resources depend on the output length: drop them, they are re-made lazily
-    for (int f = 0; f < 2; ++f) {
-        if (p->have_c2r[f]) { cufftDestroy(p->c2r[f]); p->have_c2r[f] = false; }
-        if (p->have_c2r_tail[f]) { cufftDestroy(p->c2r_tail[f]); p->have_c2r_tail[f] = false; }
-    }
-    if (p->Y) {
-        cudaFree(p->Y);
-        p->scratch_bytes -= (size_t)p->y_rows * p->ypitch * sizeof(float2);
-        p->Y = nullptr;
-    }
-    p->c2r_tail_batch = 0;
+    // the TIME-mode resources depend on the output length: drop them, they are re-made by
+    // fdd_plan_prepare or the next TIME execute
+    drop_time_resources(p);
     p->log2_dec = log2_factor;
     p->nfft_out = p->nfft >> log2_factor;
     p->nbins_out = p->nfft_out / 2 + 1;
@@ -745,6 +790,42 @@ int fdd_plan_set_kernel(fdd_plan* p, int kernel)
     if (kernel == FDD_KERNEL_SYMMETRIC2 && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     p->kernel_request = kernel;
     p->kernel = resolve_kernel(p, kernel);
+    return FDD_OK;
+}
+
+int fdd_plan_set_y_budget(fdd_plan* p, size_t bytes)
+{
+    if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
+    drop_time_resources(p);
+    p->y_budget = bytes;
+    return FDD_OK;
+}
+
+int fdd_plan_prepare(fdd_plan* p, int mode)
+{
+    if (check_plan(p) != FDD_OK || (mode != FDD_MODE_TIME && mode != FDD_MODE_FOURIER))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    int rc;
+    int family = 0;
+    if (mode == FDD_MODE_TIME && (rc = ensure_time_family(p, &family)) != FDD_OK) return rc;
+    // the bin-recurrence tables, if any DM row can reach the generic kernel
+    const bool generic_rows = p->kernel == FDD_KERNEL_GENERIC || p->kernel == FDD_KERNEL_MIXED ||
+                              (mode == FDD_MODE_TIME && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0);
+    if (generic_rows && p->rec_pshift >= 0 && (rc = ensure_rec_tables(p, nullptr)) != FDD_OK) return rc;
+    // launch shapes of the shared-recurrence kernel for the chunks an execute will step through
+    if (p->kernel == FDD_KERNEL_SYMMETRIC2) {
+        const int step = mode == FDD_MODE_TIME ? p->y_rows : p->ndm;
+        for (int j0 = 0; j0 < p->ndm && step % fdd::kSymT == 0; j0 += step) {
+            const int rows = p->ndm - j0 < step ? p->ndm - j0 : step;
+            if (!p->sym2_shapes.count(std::make_pair(j0, rows)))
+                p->sym2_shapes.emplace(std::make_pair(j0, rows), fdd::sym2_shape(p->sym, j0, rows));
+        }
+    }
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return FDD_ERR_CUDA; }
     return FDD_OK;
 }
 
@@ -792,7 +873,8 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
     // The device side of the output is a ring of kHostRingChunks chunks (Algorithm 1's output
     // buffers): results may be larger than HBM, only the host array holds them all.
     int rc;
-    if (mode == FDD_MODE_TIME && (rc = ensure_time_resources(p)) != FDD_OK) return rc;
+    int family = 0;
+    if (mode == FDD_MODE_TIME && (rc = ensure_time_family(p, &family)) != FDD_OK) return rc;
     // chunk = what run_post will step by: kHostChunkRows, or the whole Y scratch if that is smaller
     const int chunk = (mode == FDD_MODE_TIME && p->y_rows < kHostChunkRows) ? p->y_rows : kHostChunkRows;
     const int ring_rows = kHostRingChunks * chunk;

@@ -53,7 +53,10 @@ k_rotate_sum_generic(const float2* __restrict__ X, long long xpitch,
         const unsigned long long* prow = phase64 + (long long)c * ndm_pad + j0;
 #pragma unroll
         for (int i = 0; i < kGenDT; ++i) {
-            const float ph = phase_cycles_from_fixed(__ldg(prow + i), (unsigned int)kk);
+            // (a DM tile that starts off the 8-DM grid may reach past the padded row: clamp;
+            //  those trial DMs are >= ndm and never stored)
+            const int ii = j0 + i < ndm_pad ? i : ndm_pad - 1 - j0;
+            const float ph = phase_cycles_from_fixed(__ldg(prow + ii), (unsigned int)kk);
             float s, co;
             __sincosf(ph * two_pi, &s, &co);
             acc[i].x = fmaf(x.x, co, acc[i].x);

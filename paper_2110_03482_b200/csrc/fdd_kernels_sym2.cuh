@@ -365,20 +365,55 @@ inline int sym2_group(const SymTables& t, int tile0, int ntl, int ns, std::vecto
     return (int)start->size();
 }
 
+// The launch shape of rows [j_begin, j_begin + rows): sub-tiles per CTA group (NS) and the group
+// lists, one per launch of at most kSym2MaxGroups groups.  Made once per chunk at plan time /
+// first use and kept by the plan, so a launch allocates nothing.
+struct Sym2Shape {
+    int ns = 3;
+    std::vector<Sym2Groups> groups;
+    std::vector<int> ngroups;
+};
+
+inline Sym2Shape sym2_shape(const SymTables& t, int j_begin, int rows)
+{
+    Sym2Shape sh;
+    const int tile0 = j_begin / kSymT;
+    const int ntl = (rows + kSymT - 1) / kSymT;
+    std::vector<unsigned short> gs3, gs2;
+    std::vector<unsigned char> gc3, gc2;
+    // 96-DM groups (NS = 3) unless 64-DM groups leave fewer sub-tiles idle: measured cost of one
+    // group per (channel, warp): 294 cycles for NS = 3, 232 for NS = 2
+    const long long cost3 = 294LL * sym2_group(t, tile0, ntl, 3, &gs3, &gc3);
+    const long long cost2 = 232LL * sym2_group(t, tile0, ntl, 2, &gs2, &gc2);
+    sh.ns = cost3 <= cost2 ? 3 : 2;
+    const std::vector<unsigned short>& gs = sh.ns == 3 ? gs3 : gs2;
+    const std::vector<unsigned char>& gc = sh.ns == 3 ? gc3 : gc2;
+    const int all = (int)gs.size();
+    for (int g0 = 0; g0 < all; g0 += kSym2MaxGroups) {
+        const int n = all - g0 < kSym2MaxGroups ? all - g0 : kSym2MaxGroups;
+        Sym2Groups g;
+        for (int i = 0; i < kSym2MaxGroups; ++i) {
+            g.start[i] = i < n ? gs[g0 + i] : 0;
+            g.count[i] = i < n ? gc[g0 + i] : 0;
+        }
+        sh.groups.push_back(g);
+        sh.ngroups.push_back(n);
+    }
+    return sh;
+}
+
 // Rows [j_begin, j_begin + rows) -> dst[(j - j_begin) * opitch + k]; j_begin a multiple of kSymT.
 template <int NS, int kMinCtas>
-inline int sym2_launch(bool mirror, long long nfft, const SymTables& t, const float2* X, long long xpitch, int nchans,
-                       long long nbins, int ndm, int j_begin, int rows, float2* dst,
-                       long long opitch, float scale, int real_edges, float dc_add, cudaStream_t s)
+inline int sym2_launch(const Sym2Shape& sh, bool mirror, long long nfft, const SymTables& t, const float2* X,
+                       long long xpitch, int nchans, long long nbins, int ndm, int j_begin, int rows,
+                       float2* dst, long long opitch, float scale, int real_edges, float dc_add,
+                       cudaStream_t s)
 {
-    if (j_begin % kSymT != 0 || !t.centre64) return -5;
+    if (j_begin % kSymT != 0 || !t.centre64 || sh.ns != NS) return -5;
     const int tile0 = j_begin / kSymT;
     const int ntl = (rows + kSymT - 1) / kSymT;
     if (ntl > 65535) return -5;
     const int row_end = j_begin + rows < ndm ? j_begin + rows : ndm;
-    std::vector<unsigned short> gstart;
-    std::vector<unsigned char> gcount;
-    const int ngroups_all = sym2_group(t, tile0, ntl, NS, &gstart, &gcount);
     // mirror: 64 bin pairs (k, N/2 - k), k = 0 .. N/4, per CTA
     const long long nkb = mirror ? ((nbins - 1) / 2 + 1 + kSym2Threads / 2 - 1) / (kSym2Threads / 2)
                                  : (nbins + kSym2Threads - 1) / kSym2Threads;
@@ -389,13 +424,9 @@ inline int sym2_launch(bool mirror, long long nfft, const SymTables& t, const fl
     k_rotate_sum_sym2<NS, kMinCtas, MODE, MIRROR><<<grid, kSym2Threads, 0, s>>>(                   \
         X, xpitch, t.centre64, t.half64, nchans, nbins, tile0, ngroups, groups, row_end, dst,      \
         opitch, j_begin, scale, real_edges, dc_add, pshift)
-    for (int g0 = 0; g0 < ngroups_all; g0 += kSym2MaxGroups) {     // one launch per 256 groups
-        const int ngroups = ngroups_all - g0 < kSym2MaxGroups ? ngroups_all - g0 : kSym2MaxGroups;
-        Sym2Groups groups;
-        for (int g = 0; g < kSym2MaxGroups; ++g) {
-            groups.start[g] = g < ngroups ? gstart[g0 + g] : 0;
-            groups.count[g] = g < ngroups ? gcount[g0 + g] : 0;
-        }
+    for (size_t l = 0; l < sh.groups.size(); ++l) {                // one launch per 256 groups
+        const int ngroups = sh.ngroups[l];
+        const Sym2Groups& groups = sh.groups[l];
         if ((long long)ngroups * nkb > 2147483647LL) return -5;
         const unsigned grid = (unsigned)(ngroups * nkb);
         if (mirror) {

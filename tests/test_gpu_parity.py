@@ -352,6 +352,60 @@ def test_execute_host_output_ring_wraps(F):
             assert np.array_equal(got[:384], dev[:384])
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("budget_rows", [20, 32, 100, 400])
+def test_dm_chunked_time_path(F, budget_rows, kernel):
+    """TIME mode with a Y scratch smaller than the plan (fdd_plan_set_y_budget): a4 + a5 run chunk
+    after chunk - 16-row chunks off the 32-DM tiling (generic kernel, C2R), one 32-DM tile, 96-DM
+    groups, 384-row batches + a 72-row tail - through fdd_execute and fdd_execute_host."""
+    import torch
+    w = synth.small_workload(41, 24, 2048, 456, dm_step=0.11)        # ndm a multiple of 8
+    u8 = synth.make_filterbank(w)
+    ref = O.fdd_fft(u8, _delays_for(w), mode="time")
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        plan.set_y_budget(budget_rows * 1040 * 8)                     # rows of 1025 -> 1040 float2
+        plan.prepare(F.FDD_MODE_TIME)
+        got = _run(F, plan, u8, "time")
+        parity.assert_rows(got, ref, "time", f"chunked {budget_rows}/{kernel}")
+        h_out = torch.full((plan.ndm, plan.nsamps), float("nan"), dtype=torch.float32).pin_memory()
+        plan.execute_host(u8, h_out, F.FDD_MODE_TIME)
+        parity.assert_rows(h_out.numpy(), ref, "time", f"chunked host {budget_rows}/{kernel}")
+        plan.set_y_budget(0)
+        parity.assert_rows(_run(F, plan, u8, "time"), ref, "time", "default budget again")
+        plan.set_y_budget(3 * 1040 * 8)                               # not even 8 rows
+        with pytest.raises(F.FddError):
+            _run(F, plan, u8, "time")
+
+
+@pytest.mark.parametrize("kernel", ["auto", "generic"])
+@pytest.mark.parametrize("mode", ["time", "fourier"])
+def test_prepared_execute_is_captured_in_a_cuda_graph(F, mode, kernel):
+    """After fdd_plan_prepare an execute allocates nothing and never synchronises (include/fdd.h):
+    it can be captured in a CUDA graph, and the replay gives the oracle's rows."""
+    import torch
+    w = synth.small_workload(43, 32, 4096, 70, dm_step=0.4, mode=mode)
+    u8 = synth.make_filterbank(w)
+    ref = O.fdd_fft(u8, _delays_for(w), mode=mode)
+    m = F.FDD_MODE_TIME if mode == "time" else F.FDD_MODE_FOURIER
+    d_in = torch.from_numpy(u8).cuda()
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        shape = (plan.ndm, plan.nsamps) if mode == "time" else (plan.ndm, plan.nbins, 2)
+        out = torch.zeros(shape, dtype=torch.float32, device="cuda")
+        plan.prepare(m)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):                   # the first execute of this plan, under capture
+            plan.execute(d_in, out, m, torch.cuda.current_stream())
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        if mode == "fourier":
+            got = got[..., 0] + 1j * got[..., 1]
+    parity.assert_rows(got, ref, mode, f"graph replay/{mode}/{kernel}")
+
+
 def test_streams_determinism_and_plan_churn(F):
     """Executes on a non-default stream, repeated executes are bit-identical (no atomics, fixed
     summation order), and creating / destroying plans gives the device memory back."""
@@ -395,6 +449,9 @@ def test_stage_profile_and_errors(F):
             plan.execute(torch.zeros(4, device="cuda"), 0, F.FDD_MODE_TIME)     # NULL out
         with pytest.raises(F.FddError):
             plan.execute(torch.zeros(4, device="cuda"), torch.zeros(4, device="cuda"), 7)
+    # delays longer than the series: nothing is valid (not a negative length)
+    with F.Plan.create_from_delays(2, 64, np.array([[0.0, 0.0], [100.0, 3.0]])) as plan:
+        assert plan.get_info()[2] == 0
     tf, ms_ = F.measure_fp32_peak(True, 256)
     assert tf > 1.0
 

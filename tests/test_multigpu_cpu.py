@@ -74,3 +74,16 @@ def test_dm_block_sharding_world2():
     full = O.fdd_fft(u8, d, mode="time")[:, :64]
     got = np.concatenate([r[3] for r in res], axis=0)
     assert np.abs(got - full).max() <= 1e-9 * np.abs(full).max()
+
+
+def test_bench_gpus_n_starts_n_ranks_or_fails_loudly():
+    """`python bench.py --gpus 2` outside torchrun must start 2 ranks itself; on a box with fewer
+    than 2 GPUs (this one has none) it must refuse, never run one rank and call it two."""
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE")}
+    if torch.cuda.device_count() >= 2:
+        return                                   # on a multi-GPU box the GPU suite covers the launch
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1",
+                        "--warmup", "1"], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "CUDA device(s) are visible" in (r.stderr + r.stdout)
+    assert '"n_gpus"' not in r.stdout
