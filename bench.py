@@ -57,7 +57,7 @@ def parse_args():
                     choices=["tiny", "config2", "config3", "config4", "config5", "paper"])
     ap.add_argument("--ndm", type=int, default=None, help="trial DMs (config 4 sweep point)")
     ap.add_argument("--kernel", default="auto",
-                    choices=["auto", "generic", "symmetric", "symmetric2"])
+                    choices=["auto", "generic", "symmetric", "symmetric2", "tensor"])
     ap.add_argument("--decimate", type=int, default=0, metavar="M",
                     help="row f3: reduced-length inverse transform, output down-sampled by 2^M "
                          "(PAPER.md:98); the rate still counts the INPUT samples dedispersed")
@@ -305,7 +305,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     plan = F.Plan.create(w.nchans, w.nsamps, w.tsamp, w.f_lo, w.f_hi, w.dm_list)
     plan.set_kernel({"auto": F.FDD_KERNEL_AUTO, "generic": F.FDD_KERNEL_GENERIC,
                      "symmetric": F.FDD_KERNEL_SYMMETRIC,
-                     "symmetric2": F.FDD_KERNEL_SYMMETRIC2}[args.kernel])
+                     "symmetric2": F.FDD_KERNEL_SYMMETRIC2,
+                     "tensor": F.FDD_KERNEL_TENSOR}[args.kernel])
     nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
     if args.decimate:
         plan.set_decimation(args.decimate)
@@ -456,6 +457,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
                                   111 * 2 / 96.0 if ns3 else 79 * 2 / 64.0),
         F.FDD_KERNEL_MIXED: ("k_rotate_sum_sym2 + k_rotate_sum_krec (mixed)", 111 * 2 / 96.0),
         F.FDD_KERNEL_SYMMETRIC: ("k_rotate_sum_sym", 47 * 2 / 32.0),
+        F.FDD_KERNEL_TENSOR: ("k_rotate_sum_tc", 0.0),
         # bin-recurrence kernel: 4 FMA for the MAC + 4 for the advance on 7 of 8 bins
         F.FDD_KERNEL_GENERIC: ("k_rotate_sum_krec", 7.5) if nfft <= (1 << 23)
         else ("k_rotate_sum_generic", 4.0)}[kernel]

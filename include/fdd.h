@@ -74,9 +74,14 @@ enum fdd_kernel {
     FDD_KERNEL_SYMMETRIC2 = 3, /* same, up to three adjacent 32-DM tiles per CTA sharing one phasor
                                   recurrence; the groups follow the uniform segments of the DM
                                   plan (a group ends where the DM step changes)                  */
-    FDD_KERNEL_MIXED = 4       /* SYMMETRIC2 for the 32-DM tiles that are arithmetic progressions,
+    FDD_KERNEL_MIXED = 4,      /* SYMMETRIC2 for the 32-DM tiles that are arithmetic progressions,
                                   GENERIC for the few that are not (a DM plan whose step changes
                                   inside a tile)                                                */
+    FDD_KERNEL_TENSOR = 5      /* uniform DM grids (ONE arithmetic progression over all trial DMs),
+                                  <= 1024 channels, nfft <= 2^23: per Fourier bin the sum is a real
+                                  matrix product over the channels (tile-centre rotated spectra x
+                                  pair phasors), run on the tcgen05 tensor cores with fp16 hi + lo
+                                  operands and fp32 accumulation in TMEM           */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */
@@ -226,6 +231,11 @@ int fdd_rotate_sum_only(fdd_plan *plan, void *out, int mode, void *cuda_stream);
  * denominator of the a4 roofline).  packed != 0 uses fma.rn.f32x2.  Writes
  * TFLOP/s (2 flop per FMA lane) and the kernel time.  Synchronous. */
 int fdd_measure_fp32_peak(int packed, int iters, double *tflops_host, float *ms_host);
+
+/* Self-test of the tensor-core path's conventions: d_dev[128][64] (float, DEVICE) = A * B^T for
+ * a_f16_dev[128][64] and b_f16_dev[64][64] (IEEE half, row-major, DEVICE), through the shared-memory
+ * operand layout, descriptors, tcgen05.mma sequence and TMEM read-out FDD_KERNEL_TENSOR uses. */
+int fdd_tc_selftest(const void *a_f16_dev, const void *b_f16_dev, float *d_dev, void *cuda_stream);
 
 const char *fdd_error_string(int status);
 

@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "csrc", "libfdd_b200.so")
 FDD_MODE_TIME, FDD_MODE_FOURIER = 0, 1
 FDD_KERNEL_AUTO, FDD_KERNEL_GENERIC, FDD_KERNEL_SYMMETRIC, FDD_KERNEL_SYMMETRIC2 = 0, 1, 2, 3
 FDD_KERNEL_MIXED = 4
+FDD_KERNEL_TENSOR = 5
 FDD_OK = 0
 FDD_NUM_STAGES = 6
 STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift_add")
@@ -26,7 +27,8 @@ EXPORTS = (
     "fdd_plan_set_y_budget",
     "fdd_execute", "fdd_execute_host", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
-    "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_error_string",
+    "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
+    "fdd_error_string",
 )
 
 
@@ -71,6 +73,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
     lib.fdd_plan_get_spectrum.argtypes = [vp, P(vp), P(c_ll), P(c_dbl)]
     lib.fdd_rotate_sum_only.argtypes = [vp, vp, c_int, vp]
+    lib.fdd_tc_selftest.argtypes = [vp, vp, vp, vp]
     lib.fdd_measure_fp32_peak.argtypes = [c_int, c_int, P(c_dbl), P(ctypes.c_float)]
     for name in EXPORTS:
         getattr(lib, name).restype = c_int
@@ -252,3 +255,9 @@ def measure_fp32_peak(packed: bool, iters: int = 4096) -> Tuple[float, float]:
     _check(load_library().fdd_measure_fp32_peak(int(bool(packed)), int(iters), ctypes.byref(tf),
                                                 ctypes.byref(ms)), "fdd_measure_fp32_peak")
     return tf.value, ms.value
+
+
+def tc_selftest(a_f16, b_f16, d_out, stream=None) -> None:
+    """d_out[128][64] f32 = a_f16[128][64] @ b_f16[64][64].T on the tcgen05 path (device tensors)."""
+    _check(load_library().fdd_tc_selftest(_ptr(a_f16), _ptr(b_f16), _ptr(d_out), _stream_handle(stream)),
+           "fdd_tc_selftest")

@@ -19,6 +19,7 @@
 #include "fdd_kernels_pre.cuh"
 #include "fdd_kernels_sym.cuh"
 #include "fdd_kernels_sym2.cuh"
+#include "fdd_kernels_tc.cuh"
 #include "fdd_kernels_tdd.cuh"
 
 namespace {
@@ -54,6 +55,7 @@ struct fdd_plan {
     double max_delay = 0;
     long long valid_len = 0;
     int device = 0;
+    int num_sms = 0;
     float offset = 0.f;                  // subtracted by a2, restored in bin 0 by a4 (S21)
     // device buffers
     float2* X = nullptr;                 // [nchans][xpitch] spectra
@@ -166,12 +168,20 @@ void finish_delay_stats(fdd_plan* p)
     if (p->valid_len < 0) p->valid_len = 0;          // delays longer than the series: nothing is valid
 }
 
+// The tensor-core kernel needs ONE arithmetic progression over all trial DMs (a uniform DM grid), at
+// most 1024 channels (phase steps staged in shared memory) and nfft <= 2^23 (FP64-pipe phases).
+bool tensor_ok(const fdd_plan* p)
+{
+    return p->sym_ok && p->sym.pair_ok && p->nchans <= fdd::kTcMaxChans && p->rec_pshift >= 0;
+}
+
 // AUTO: the fastest kernel the delay table allows.
 int resolve_kernel(const fdd_plan* p, int request)
 {
     const bool sym2_ok = p->sym_ok;      // groups of sub-tiles follow the DM plan's uniform segments
     const bool any_ap = p->sym.nap > 0;
     switch (request) {
+        case FDD_KERNEL_TENSOR: return tensor_ok(p) ? FDD_KERNEL_TENSOR : FDD_KERNEL_GENERIC;
         case FDD_KERNEL_GENERIC: return FDD_KERNEL_GENERIC;
         case FDD_KERNEL_SYMMETRIC: return p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC;
         case FDD_KERNEL_MIXED: return sym2_ok ? FDD_KERNEL_SYMMETRIC2
@@ -435,6 +445,8 @@ int create_common(fdd_plan* p)
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return FDD_ERR_CUDA; }
     if (cudaGetDevice(&p->device) != cudaSuccess) return FDD_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess)
+        return FDD_ERR_CUDA;
     p->nfft = 2;
     while (p->nfft < p->nsamps) p->nfft <<= 1;
     p->nbins = p->nfft / 2 + 1;
@@ -523,6 +535,22 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
+    if (kernel == FDD_KERNEL_TENSOR && j_begin % fdd::kSymT == 0 && !mirror) {
+        // fp16 operands: X times a power of two such that |X| <= 255 nsamps cannot overflow them
+        int e = 0;
+        frexp((p->offset != 0.f ? 128.0 : 255.0) * (double)p->nsamps, &e);      // |X| < 2^e
+        const float xscale = (float)ldexp(1.0, 15 - e);
+        const int per = fdd::kTcT * (fdd::kTcRows / 2);                          // trial DMs per launch
+        for (int r0 = 0; r0 < rows; r0 += per) {
+            const int n = rows - r0 < per ? rows - r0 : per;
+            const int rc = fdd::tc_launch(p->sym, p->nfft, p->X, p->xpitch, p->nchans, p->nbins_out, p->ndm,
+                                          j_begin + r0, n, dst + (long long)r0 * opitch, opitch, scale,
+                                          real_edges, dc_add, xscale, p->num_sms, s);
+            if (rc != 0) return rc;
+        }
+        return FDD_OK;
+    }
+    if (kernel == FDD_KERNEL_TENSOR) kernel = FDD_KERNEL_SYMMETRIC2;   // (a chunk off the 32-DM tiling)
     if (kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
         // the grouping of the chunk's 32-DM sub-tiles is made once per (first row, rows)
         auto it = p->sym2_shapes.find(std::make_pair(j_begin, rows));
@@ -784,7 +812,8 @@ int fdd_plan_get_output_shape(const fdd_plan* p, long long* nsamps_out, long lon
 int fdd_plan_set_kernel(fdd_plan* p, int kernel)
 {
     if (check_plan(p) != FDD_OK) return FDD_ERR_INVALID_ARG;
-    if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_MIXED) return FDD_ERR_INVALID_ARG;
+    if (kernel < FDD_KERNEL_AUTO || kernel > FDD_KERNEL_TENSOR) return FDD_ERR_INVALID_ARG;
+    if (kernel == FDD_KERNEL_TENSOR && !tensor_ok(p)) return FDD_ERR_UNSUPPORTED;
     if (kernel == FDD_KERNEL_MIXED && p->sym.nap == 0) return FDD_ERR_UNSUPPORTED;
     if (kernel == FDD_KERNEL_SYMMETRIC && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     if (kernel == FDD_KERNEL_SYMMETRIC2 && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
@@ -979,6 +1008,19 @@ int fdd_tdd_execute(fdd_plan* p, const unsigned char* in_u8, float* out, void* c
         p->tdd_xt, p->tdd_tpitch, p->tdd_shifts, p->ndm_pad, p->nchans, p->nsamps, p->ndm, ntiles_dm,
         out);
     tm.end();
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
+int fdd_tc_selftest(const void* a_f16_dev, const void* b_f16_dev, float* d_dev, void* cuda_stream)
+{
+    if (!a_f16_dev || !b_f16_dev || !d_dev) return FDD_ERR_INVALID_ARG;
+    const int smem = 1024 + fdd::kTcZBytes + fdd::kTcEBytes + 64;
+    if (cudaFuncSetAttribute(fdd::k_tc_selftest, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
+        cudaGetLastError();
+        return FDD_ERR_CUDA;
+    }
+    fdd::k_tc_selftest<<<1, 128, smem, static_cast<cudaStream_t>(cuda_stream)>>>(
+        static_cast<const __half*>(a_f16_dev), static_cast<const __half*>(b_f16_dev), d_dev);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 

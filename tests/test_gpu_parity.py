@@ -630,3 +630,41 @@ def test_full_size_integer_delays(F, table):
     # sums of 1024 bytes reach 1.3e5 where the fp32 ulp is 1/64: the rounded value is the integer
     assert np.abs(got - ref).max() <= 0.25
     assert np.array_equal(np.rint(got).astype(np.int64), ref)
+
+
+# ------------------------------------------------------------------ tensor-core kernel (tcgen05)
+def test_tensor_core_conventions_selftest(F):
+    """fdd_tc_selftest: fp16 A[128][64] B[64][64] -> A B^T through the operand layout, descriptors,
+    tcgen05.mma sequence and TMEM read-out of FDD_KERNEL_TENSOR; the reference is a numpy matmul of
+    the same fp16 values in fp64 (products of fp16 values are exact in fp32: only the summation
+    order differs)."""
+    import torch
+    rng = np.random.default_rng(17)
+    a = rng.standard_normal((128, 64)).astype(np.float16)
+    b = rng.standard_normal((64, 64)).astype(np.float16)
+    d = torch.zeros((128, 64), dtype=torch.float32, device="cuda")
+    F.tc_selftest(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), d)
+    torch.cuda.synchronize()
+    ref = a.astype(np.float64) @ b.astype(np.float64).T
+    assert np.abs(d.cpu().numpy() - ref).max() <= 2e-5 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("mode", ["time", "fourier"])
+@pytest.mark.parametrize("nchans,nsamps,ndm,step", [
+    (64, 8192, 32, None),            # config-1 shape on a one-sample grid: half a tile
+    (100, 4096, 200, 0.3),           # ragged channels (two 64-channel stages, 28 padded), 3 tiles + 8 rows
+    (256, 1000, 4096, 0.02),         # all 64 tiles, padded series (1000 -> 1024), last item 1 live bin
+    (1024, 2048, 300, 0.05),         # the most channels the kernel stages
+])
+def test_tensor_core_kernel_against_the_oracle(F, oracle_c, nchans, nsamps, ndm, step, mode):
+    w = synth.small_workload(600 + nchans, nchans, nsamps, ndm, dm_step=step, mode=mode)
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = list(range(ndm)) if ndm <= 300 else sorted(set(range(0, ndm, 61)) | {31, 32, 63, 64, ndm - 1})
+    ref = O.fdd_rows(u8, d, rows, mode=mode)
+    with _plan_for(F, w) as plan:
+        plan.set_kernel(F.FDD_KERNEL_TENSOR)
+        assert plan.get_info()[5] == F.FDD_KERNEL_TENSOR
+        got = _run(F, plan, u8, mode)[rows]
+    worst = parity.assert_rows(got, ref, mode, f"tensor {nchans}x{nsamps}x{ndm}/{mode}")
+    print("tensor", nchans, nsamps, ndm, mode, worst)
