@@ -30,6 +30,7 @@ constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per
 constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
 constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
+constexpr int kTensorMinRows = 1024;                  // launches with fewer trial DMs take the FP32 kernels
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
@@ -187,6 +188,10 @@ int resolve_kernel(const fdd_plan* p, int request)
         case FDD_KERNEL_MIXED: return sym2_ok ? FDD_KERNEL_SYMMETRIC2
                                               : (any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC);
         default:
+            // measured on B200 (1024 channels x 2^20 samples): the tensor-core kernel costs the same
+            // for any number of trial DMs up to 4096 per launch (43 ms), the shared-recurrence kernel
+            // 46 ms per 1024 trial DMs
+            if (tensor_ok(p) && p->ndm >= kTensorMinRows) return FDD_KERNEL_TENSOR;
             if (sym2_ok) return FDD_KERNEL_SYMMETRIC2;
             // a few tiles hold a change of DM step: those rows alone take the generic kernel
             return 2 * p->sym.nap >= p->sym.ntiles && any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC;
@@ -535,7 +540,9 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
-    if (kernel == FDD_KERNEL_TENSOR && j_begin % fdd::kSymT == 0 && !mirror) {
+    // (AUTO sends short chunks to the FP32 kernel; an explicit FDD_KERNEL_TENSOR request does not)
+    if (kernel == FDD_KERNEL_TENSOR && j_begin % fdd::kSymT == 0 && !mirror &&
+        rows >= (p->kernel_request == FDD_KERNEL_TENSOR ? 1 : kTensorMinRows)) {
         // fp16 operands: X times a power of two such that |X| <= 255 nsamps cannot overflow them
         int e = 0;
         frexp((p->offset != 0.f ? 128.0 : 255.0) * (double)p->nsamps, &e);      // |X| < 2^e
@@ -550,7 +557,7 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
         }
         return FDD_OK;
     }
-    if (kernel == FDD_KERNEL_TENSOR) kernel = FDD_KERNEL_SYMMETRIC2;   // (a chunk off the 32-DM tiling)
+    if (kernel == FDD_KERNEL_TENSOR) kernel = FDD_KERNEL_SYMMETRIC2;   // (a short chunk, or one off the 32-DM tiling)
     if (kernel == FDD_KERNEL_SYMMETRIC2 && j_begin % fdd::kSymT == 0) {
         // the grouping of the chunk's 32-DM sub-tiles is made once per (first row, rows)
         auto it = p->sym2_shapes.find(std::make_pair(j_begin, rows));
