@@ -7,6 +7,7 @@
 #include <cufft.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <map>
@@ -185,6 +186,7 @@ int resolve_kernel(const fdd_plan* p, int request)
         case FDD_KERNEL_TENSOR: return tensor_ok(p) ? FDD_KERNEL_TENSOR : FDD_KERNEL_GENERIC;
         case FDD_KERNEL_GENERIC: return FDD_KERNEL_GENERIC;
         case FDD_KERNEL_SYMMETRIC: return p->sym_ok ? FDD_KERNEL_SYMMETRIC : FDD_KERNEL_GENERIC;
+        case FDD_KERNEL_SYMMETRIC2: return sym2_ok ? FDD_KERNEL_SYMMETRIC2 : FDD_KERNEL_GENERIC;
         case FDD_KERNEL_MIXED: return sym2_ok ? FDD_KERNEL_SYMMETRIC2
                                               : (any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC);
         default:
@@ -343,7 +345,9 @@ int ensure_time_resources(fdd_plan* p, int family)
                                       : (rows >= 96 ? rows / 96 * 96 : (rows >= 32 ? 32 : rows / 8 * 8));
         if (rows < 1) return FDD_ERR_ALLOC;
         p->y_rows = (int)rows;
-        p->c2r_batch = p->y_rows < kC2RBatch ? p->y_rows : kC2RBatch;
+        int batch = kC2RBatch;
+        if (const char* e = getenv("FDD_C2R_BATCH")) { const int v = atoi(e); if (v > 0) batch = v; }
+        p->c2r_batch = p->y_rows < batch ? p->y_rows : batch;
         // tails: of a full Y chunk and of the last (short) chunk; at most one distinct tail size
         const int last_rows = p->ndm % p->y_rows ? p->ndm % p->y_rows : p->y_rows;
         int tail = last_rows % p->c2r_batch;

@@ -137,7 +137,7 @@ def test_ragged_shapes(F, nchans, nsamps, ndm, step, dm0, mode, kernel):
     with _plan_for(F, w) as plan:
         _set_kernel(F, plan, kernel)
         got = _run(F, plan, u8, mode)
-        assert plan.get_info()[2] == O.valid_length(d, nsamps)
+        assert plan.get_info()[2] == max(0, O.valid_length(d, nsamps))   # (the library clamps at 0)
     if nsamps >= 256:
         parity.assert_rows(got, ref, mode, f"ragged {nchans}x{nsamps}x{ndm}/{mode}/{kernel}")
     else:
@@ -499,6 +499,7 @@ def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None):
     """One full-size TIME execute at `ndm` trial DMs; sampled rows against the oracle."""
     import torch
     w = synth.workload(name, ndm=ndm)
+    torch.cuda.empty_cache()
     _, u8 = _FullSize.input(name)
     Y = _FullSize.spectrum_rows(name, w, rows)
     ref = O.rows_from_spectrum(Y, O.next_pow2(w.nsamps), w.nsamps, "time", decimate)
@@ -607,6 +608,7 @@ def test_paper_workload_at_its_own_shape(F, oracle_c):
     d = _delays_for(w)
     rows = [0, 1, 31, 64, 96, 127]
     ref = O.fdd_rows(u8, d, rows, mode="time")
+    torch.cuda.empty_cache()                 # the plan holds 2 x 34 GB + cuFFT workspace: give back torch's cache
     with _plan_for(F, w) as plan:
         assert plan.nfft == 1 << 23 and plan.get_info()[5] == F.FDD_KERNEL_SYMMETRIC2
         d_in = torch.from_numpy(u8).cuda()
