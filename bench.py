@@ -64,6 +64,9 @@ def parse_args():
     ap.add_argument("--with-tdd", action="store_true",
                     help="row f4: also time the time-domain comparator (fdd_tdd_execute) on the "
                          "same input and report it as tdd_comparator")
+    ap.add_argument("--beams", type=int, default=1, metavar="B",
+                    help="row f1: B beams per step through fdd_execute_beams (beam 0 = the workload's "
+                         "input, the others seeded noise made on the device); the rate counts all beams")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -313,10 +316,20 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     ns_out, nbins = plan.output_shape()                   # = (nsamps, nbins) at full rate
     nfft_out = nfft >> args.decimate
     d_in = torch.from_numpy(u8).cuda()
+    nbeams = max(1, args.beams)
+    if nbeams > 1:
+        beams = torch.empty((nbeams, w.nsamps, w.nchans), dtype=torch.uint8, device="cuda")
+        beams[0] = d_in
+        gen = torch.Generator(device="cuda").manual_seed(w.seed + 99)
+        for b in range(1, nbeams):
+            beams[b] = (torch.randn((w.nsamps, w.nchans), generator=gen, device="cuda") * 16 + 128
+                        ).round().clamp(0, 255).to(torch.uint8)
+        d_in = beams
+    lead = (nbeams,) if nbeams > 1 else ()
     if mode == F.FDD_MODE_TIME:
-        out = torch.empty((w.ndm, ns_out), dtype=torch.float32, device="cuda")
+        out = torch.empty(lead + (w.ndm, ns_out), dtype=torch.float32, device="cuda")
     else:
-        out = torch.empty((w.ndm, nbins, 2), dtype=torch.float32, device="cuda")
+        out = torch.empty(lead + (w.ndm, nbins, 2), dtype=torch.float32, device="cuda")
     flush = None
     if w.nsamps * w.nchans <= (1 << 28):
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -325,7 +338,10 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     def step():
         if flush is not None:
             flush.fill_(1)
-        plan.execute(d_in, out, mode, stream)
+        if nbeams > 1:
+            plan.execute_beams(d_in, out, nbeams, mode, stream)
+        else:
+            plan.execute(d_in, out, mode, stream)
 
     # FP32 FMA rate of this GPU, measured with the library's FFMA2 probe (~0.25 s, sustained)
     peak_tf, peak_ms = F.measure_fp32_peak(True, 1 << 19)
@@ -357,7 +373,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         per_rank_ms = [float(x.item()) / args.steps for x in allt]
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
-    units = float(w.ndm) * w.nsamps * world               # DM-trials x samples, all ranks
+    units = float(w.ndm) * w.nsamps * world * nbeams      # DM-trials x samples, all ranks (and beams)
     value = units / (ms_step * 1e-3)
 
     # ---- the time-domain comparator on the same input (row f4; not part of `value`) -----
@@ -385,7 +401,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
 
     # ---- end to end through the host-buffer entry point ---------------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and nbeams == 1:
         host_memory = "pinned"
         try:
             h_in = torch.from_numpy(u8).pin_memory()
@@ -503,7 +519,11 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         except Exception:
             pk = {}
         tpeak = pk.get("bf16_tflops_sustained", 1400.0)
-        nlaunch = -(-w.ndm // 4096)
+        if nbeams > 1:
+            grp = 4 if w.ndm <= 1024 else (2 if w.ndm <= 2048 else 1)
+            nlaunch = -(-nbeams // grp) * (-(-w.ndm // 4096) if grp == 1 else 1)
+        else:
+            nlaunch = -(-w.ndm // 4096)
         kpad = -(-w.nchans // 64) * 64
         bpad = -(-nbins // 4) * 4
         mma_flop = nlaunch * 3.0 * 2.0 * 128 * 64 * kpad * bpad
@@ -525,7 +545,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": dict(workload_config(w, world), decimation_log2=args.decimate),
+        "config": dict(workload_config(w, world), decimation_log2=args.decimate, beams=nbeams),
         "ms_per_step_per_rank": per_rank_ms,
         "tdd_comparator": tdd,
         "clocks": sampler.summary(),
@@ -558,6 +578,11 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     line["hbm_peak_gbs"] = hbm
     line["hbm_peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback 6650 (B200_PROFILING.md)"
 
+    if nbeams > 1:
+        line["beams"] = {"nbeams": nbeams, "ms_per_beam": ms_step / nbeams,
+                         "rotate_sum_ms_per_beam": stage_ms["rotate_sum"] / args.steps / nbeams,
+                         "what": "fdd_execute_beams: groups of 4 beams (2 above 1024 trial DMs) share one "
+                                 "tensor-core a4 launch (PAPER.md:274)"}
     if world == 1 and not args.no_cpu_baseline:
         plan.destroy()
         del d_in, out

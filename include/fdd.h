@@ -183,6 +183,21 @@ int fdd_execute(fdd_plan *plan, const unsigned char *in_u8, void *out, int mode,
 int fdd_execute_host(fdd_plan *plan, const unsigned char *in_host, void *out_host, int mode,
                      void *cuda_stream);
 
+/* Several beams (or repeated observations) of the same receiver with one plan - the paper's route to
+ * sharing the phase rotations ("reusing phase rotations ... multiple beams").
+ *   in_u8  DEVICE, uint8 [nbeams][nsamps][nchans], every beam laid out as for fdd_execute
+ *   out    DEVICE, [nbeams] outputs of fdd_execute, one after the other
+ * On a uniform DM grid with at most 2048 trial DMs and 1024 channels, groups of 4 beams (2 above 1024
+ * trial DMs) run step a4 as ONE tensor-core launch: per Fourier bin the pair phasors are generated
+ * once and contracted against the tile-centre-rotated spectra of all beams of the group (the beams
+ * take the place of further trial-DM tiles in the rows of the matrix product, FDD_KERNEL_TENSOR), so
+ * a4 costs the same for 4 beams as for 1.  Other plans run beam after beam.  Steps a2, a3 and a5 run
+ * per beam.  The group's spectra (and, in TIME mode, sums) live in plan-owned scratch allocated on the
+ * first call (which may synchronise the device).  Results equal nbeams separate fdd_execute calls up
+ * to the kernels' rounding (the kernel choice may differ). */
+int fdd_execute_beams(fdd_plan *plan, const unsigned char *in_u8, void *out, int nbeams, int mode,
+                      void *cuda_stream);
+
 /* Free everything the plan owns.  NULL is a no-op returning FDD_OK. */
 int fdd_plan_destroy(fdd_plan *plan);
 
@@ -216,13 +231,22 @@ int fdd_plan_set_profiling(fdd_plan *plan, int enable);
 int fdd_plan_get_stage_ms(fdd_plan *plan, float *ms_host, int *launches_host);
 
 /* Debug/test access: DEVICE pointer to the channel spectra X (float2 [nchans][pitch]) left by
- * the last execute, and the row pitch in float2 elements.  When nsamps is a power of two the
- * unpack step subtracts 128 from every sample (exact) so that the mean of unsigned-byte data
- * stays out of the fp32 FFTs; the sum kernel restores it in bin 0.  *dc_removed (may be NULL)
- * receives what has to be added to Re X[c][0] of every channel to get the plain DFT
- * (128 * nsamps, or 0 when the input is zero padded). */
+ * the last execute, and the row pitch in float2 elements.  The unpack step subtracts 128 from every
+ * sample (exact) so that the mean of unsigned-byte data stays out of the fp32 FFTs; *dc_removed (may
+ * be NULL) receives what has to be added to Re X[c][0] of every channel to get the plain DFT
+ * (128 * nsamps).  When nsamps is a power of two that is all: the sum kernel restores it in bin 0.
+ * When the series is zero padded the removed mean is a rectangle, not a constant: its spectrum
+ * 128 R[k], R[k] = sum_{n < nsamps} e^{-2 pi i k n / nfft}, is missing from bins k < exact_bins of X
+ * (fdd_plan_get_padding; 4096, or all bins of a shorter spectrum) and already added back (closed form,
+ * fp64) in the bins above; the lowest bins' share of every trial DM is tabulated per plan in fp64 and
+ * added after step a4 (fdd_plan_prepare builds the table, else the first execute).  Results are those
+ * of the zero-padded series (reading S9); only the fp32 rounding differs. */
 int fdd_plan_get_spectrum(const fdd_plan *plan, void **x_dev, long long *pitch_elems,
                           double *dc_removed);
+
+/* *exact_bins = number of lowest bins whose rectangle term is handled by the per-plan table (0 when
+ * nsamps is a power of two). */
+int fdd_plan_get_padding(const fdd_plan *plan, long long *exact_bins);
 
 /* Run only a4 on the spectra left by the last execute (for timing sweeps of the hot kernel). */
 int fdd_rotate_sum_only(fdd_plan *plan, void *out, int mode, void *cuda_stream);

@@ -345,3 +345,17 @@ def single_bins(in_u8: np.ndarray, delays: np.ndarray, bins: Sequence[int],
     if rows is not None:
         d = d[list(rows)]
     return phase_rotate_sum_c(X, d, n, bins=bins)
+
+
+# ----------------------------------------------------------------------------- next row f1
+def fdd_beams(in_u8_beams: np.ndarray, delays: np.ndarray, rows: Optional[Iterable[int]] = None,
+              mode: str = "time") -> np.ndarray:
+    """Several beams with one delay table ("reusing phase rotations ... multiple
+    beams"): the beams share nothing but the phasors, so the definition is O1..O6 beam by beam.
+
+    ``in_u8_beams`` is [nbeams][nsamps][nchans]; returns [nbeams][rows][...] (at-scale tier).
+    """
+    in_u8_beams = np.asarray(in_u8_beams)
+    assert in_u8_beams.ndim == 3
+    rows = list(range(np.asarray(delays).shape[0])) if rows is None else list(rows)
+    return np.stack([fdd_rows(b, delays, rows, mode=mode) for b in in_u8_beams])

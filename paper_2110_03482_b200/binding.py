@@ -25,9 +25,9 @@ EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
     "fdd_plan_set_decimation", "fdd_plan_get_output_shape", "fdd_plan_prepare",
     "fdd_plan_set_y_budget",
-    "fdd_execute", "fdd_execute_host", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
+    "fdd_execute", "fdd_execute_host", "fdd_execute_beams", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
-    "fdd_plan_get_spectrum", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
+    "fdd_plan_get_spectrum", "fdd_plan_get_padding", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
     "fdd_error_string",
 )
 
@@ -59,6 +59,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_set_kernel.argtypes = [vp, c_int]
     lib.fdd_execute.argtypes = [vp, vp, vp, c_int, vp]
     lib.fdd_execute_host.argtypes = [vp, vp, vp, c_int, vp]
+    lib.fdd_execute_beams.argtypes = [vp, vp, vp, c_int, c_int, vp]
     lib.fdd_tdd_execute.argtypes = [vp, vp, vp, vp]
     lib.fdd_plan_destroy.argtypes = [vp]
     lib.fdd_plan_get_info.argtypes = [vp, P(c_ll), P(c_ll), P(c_ll), P(c_dbl),
@@ -73,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
     lib.fdd_plan_get_spectrum.argtypes = [vp, P(vp), P(c_ll), P(c_dbl)]
     lib.fdd_rotate_sum_only.argtypes = [vp, vp, c_int, vp]
+    lib.fdd_plan_get_padding.argtypes = [vp, P(c_ll)]
     lib.fdd_tc_selftest.argtypes = [vp, vp, vp, vp]
     lib.fdd_measure_fp32_peak.argtypes = [c_int, c_int, P(c_dbl), P(ctypes.c_float)]
     for name in EXPORTS:
@@ -167,6 +169,11 @@ class Plan:
         _check(load_library().fdd_execute_host(self._h, _ptr(in_host), _ptr(out_host), int(mode),
                                                _stream_handle(stream)), "fdd_execute_host")
 
+    def execute_beams(self, in_u8, out, nbeams: int, mode: int = FDD_MODE_TIME, stream=None) -> None:
+        """Device tensors: in_u8 [nbeams][nsamps][nchans], out [nbeams][...]."""
+        _check(load_library().fdd_execute_beams(self._h, _ptr(in_u8), _ptr(out), int(nbeams), int(mode),
+                                                _stream_handle(stream)), "fdd_execute_beams")
+
     def tdd_execute(self, in_u8, out, stream=None) -> None:
         """The time-domain comparator (Eq. 2): device tensors, out float32 [ndm][nsamps]."""
         _check(load_library().fdd_tdd_execute(self._h, _ptr(in_u8), _ptr(out),
@@ -230,6 +237,12 @@ class Plan:
         _check(load_library().fdd_plan_get_spectrum(self._h, ctypes.byref(x), ctypes.byref(pitch),
                                                     ctypes.byref(dc)), "fdd_plan_get_spectrum")
         return x.value, pitch.value, dc.value
+
+    def get_padding(self) -> int:
+        """Lowest bins whose mean-rectangle term a per-plan fp64 table supplies (0: not zero padded)."""
+        n = ctypes.c_longlong()
+        _check(load_library().fdd_plan_get_padding(self._h, ctypes.byref(n)), "fdd_plan_get_padding")
+        return int(n.value)
 
     def destroy(self) -> None:
         if self._h is not None and self._h.value:

@@ -17,6 +17,7 @@
 
 #include "fdd_kernels_generic.cuh"
 #include "fdd_kernels_krec.cuh"
+#include "fdd_kernels_pad.cuh"
 #include "fdd_kernels_pre.cuh"
 #include "fdd_kernels_sym.cuh"
 #include "fdd_kernels_sym2.cuh"
@@ -59,6 +60,11 @@ struct fdd_plan {
     int device = 0;
     int num_sms = 0;
     float offset = 0.f;                  // subtracted by a2, restored in bin 0 by a4 (S21)
+    // zero-padded series (fdd_kernels_pad.cuh): the rectangle's share of the lowest bins, per plan
+    bool padded = false;
+    int pad_k = 0;                       // bins treated exactly
+    float2* pad_tab = nullptr;           // [ndm][pad_k], built by fdd_plan_prepare / on first use
+    bool pad_ready = false;
     // device buffers
     float2* X = nullptr;                 // [nchans][xpitch] spectra
     float* xreal = nullptr;              // [nchans][nfft] unpacked series (out-of-place R2C input)
@@ -93,6 +99,10 @@ struct fdd_plan {
     int c2r_batch = 0, c2r_tail_batch = 0;
     void* fft_ws = nullptr;
     size_t fft_ws_bytes = 0;
+    // multi-beam execution (fdd_execute_beams): spectra and TIME-mode sums of one group of beams
+    float2* beam_X = nullptr;            // [beam_group][nchans][xpitch]
+    float2* beam_Y = nullptr;            // [beam_group][ndm][ypitch]
+    int beam_group = 0;
     // host staging (fdd_execute_host)
     unsigned char* stage_in = nullptr;
     void* stage_out = nullptr;
@@ -215,6 +225,7 @@ int upload_generic_table(fdd_plan* p)
         cudaGetLastError();
         return FDD_ERR_CUDA;
     }
+    p->pad_ready = false;
     p->rec_ready = false;                // rebuilt by fdd_plan_prepare / the next generic launch
     p->sym2_shapes.clear();
     return FDD_OK;
@@ -315,7 +326,8 @@ int make_c2r_plan(fdd_plan* p, int family, cufftHandle* h, int batch, size_t* ws
 // spectrum the mirrored sym2 epilogue writes, 0 = cuFFT's C2R from Y.
 int time_family(const fdd_plan* p)
 {
-    return (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4) ? 1 : 0;
+    // (a zero-padded plan adds the rectangle's table to Y after a4, so a4 must write plain sums)
+    return (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4 && !p->padded) ? 1 : 0;
 }
 
 void drop_c2r_plan(cufftHandle* h, bool* have)
@@ -400,6 +412,11 @@ void drop_time_resources(fdd_plan* p)
         p->scratch_bytes -= (size_t)p->y_rows * p->ypitch * sizeof(float2);
         p->Y = nullptr;
     }
+    if (p->beam_Y) {
+        cudaFree(p->beam_Y);
+        p->scratch_bytes -= (size_t)p->beam_group * p->ndm * p->ypitch * sizeof(float2);
+        p->beam_Y = nullptr;
+    }
     p->y_rows = 0;
     p->c2r_tail_batch = 0;
     p->sym2_shapes.clear();
@@ -441,6 +458,9 @@ void destroy_plan(fdd_plan* p)
     cudaFree(p->fft_ws);
     cudaFree(p->stage_in);
     cudaFree(p->stage_out);
+    cudaFree(p->pad_tab);
+    cudaFree(p->beam_X);
+    cudaFree(p->beam_Y);
     fdd::sym_free_tables(&p->sym);
     for (auto& e : p->events) { cudaEventDestroy(e.beg); cudaEventDestroy(e.end); }
     for (auto& e : p->chunk_events) cudaEventDestroy(e);
@@ -460,8 +480,11 @@ int create_common(fdd_plan* p)
     while (p->nfft < p->nsamps) p->nfft <<= 1;
     p->nbins = p->nfft / 2 + 1;
     p->nfft_out = p->nfft; p->nbins_out = p->nbins; p->nsamps_out = p->nsamps;
-    // Without zero padding a constant offset lives in bin 0 alone; with padding it would not.
-    p->offset = p->nsamps == p->nfft ? 128.f : 0.f;
+    // The mean of unsigned-byte data stays out of the fp32 transforms.  Without zero padding it lives in
+    // bin 0 alone; with padding it is a rectangle, handled in fdd_kernels_pad.cuh.
+    p->offset = 128.f;
+    p->padded = p->nsamps != p->nfft;
+    p->pad_k = (int)(p->nbins < fdd::kPadExactBins ? p->nbins : fdd::kPadExactBins);
     p->xpitch = round_up(p->nbins, kPitchAlign);
     p->ndm_pad = (int)round_up(p->ndm, fdd::kGenDT);
     int rc = dev_alloc(p, &p->X, (size_t)p->nchans * p->xpitch);
@@ -533,6 +556,49 @@ int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
+// Zero-padded plans: the per-plan table of fdd_kernels_pad.cuh (fp64 on the device, once per plan).
+int ensure_pad_table(fdd_plan* p, cudaStream_t s)
+{
+    if (!p->padded || p->pad_ready) return FDD_OK;
+    int rc;
+    if (!p->pad_tab && (rc = dev_alloc(p, &p->pad_tab, (size_t)p->ndm * p->pad_k)) != FDD_OK) return rc;
+    dim3 grid((unsigned)((p->pad_k + 127) / 128), (unsigned)p->ndm);
+    fdd::k_pad_build_table<<<grid, 128, 0, s>>>(p->phase64, p->ndm_pad, p->nchans, p->ndm, p->pad_k, p->nsamps,
+                                                p->nfft, (double)p->offset, p->pad_tab);
+    if (cudaGetLastError() != cudaSuccess) return FDD_ERR_CUDA;
+    p->pad_ready = true;
+    return FDD_OK;
+}
+
+// after a3: the rectangle's spectrum goes back into the bins where it is no larger than the data
+int launch_pad_add_rect(fdd_plan* p, float2* X, cudaStream_t s)
+{
+    if (!p->padded || p->pad_k >= p->nbins) return FDD_OK;
+    dim3 grid((unsigned)((p->nbins - p->pad_k + 255) / 256), (unsigned)((p->nchans + 31) / 32));
+    fdd::k_pad_add_rect<<<grid, 256, 0, s>>>(X, p->xpitch, p->nchans, p->pad_k, p->nbins, p->nsamps, p->nfft,
+                                             (double)p->offset);
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
+// after a4: ... and into the lowest bins of the sums, from the table
+int launch_pad_add_table(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
+                         cudaStream_t s)
+{
+    if (!p->padded) return FDD_OK;
+    int rc = ensure_pad_table(p, s);
+    if (rc != FDD_OK) return rc;
+    const int kuse = (int)(p->pad_k < p->nbins_out ? p->pad_k : p->nbins_out);
+    const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
+    for (int r0 = 0; r0 < rows; r0 += 32768) {
+        const int n = rows - r0 < 32768 ? rows - r0 : 32768;
+        dim3 grid((unsigned)((kuse + 255) / 256), (unsigned)n);
+        fdd::k_pad_add_table<<<grid, 256, 0, s>>>(dst + (long long)r0 * opitch, opitch, p->pad_tab, p->pad_k, kuse,
+                                                  j_begin + r0, n, scale, mode == FDD_MODE_TIME ? 1 : 0,
+                                                  p->nbins_out);
+    }
+    return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
+}
+
 // a4 on DM rows [j_begin, j_begin + rows) into dst (row pitch opitch float2).
 // mirror (SYMMETRIC2, TIME mode only): dst receives the pre-twiddled Z of the half-length inverse
 // transform instead of Y (fdd_kernels_sym2.cuh).
@@ -542,14 +608,14 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
     const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
-    const double dc_raw = (double)p->offset * (double)p->nchans * (double)p->nsamps;
+    const double dc_raw = p->padded ? 0.0 : (double)p->offset * (double)p->nchans * (double)p->nsamps;
     const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
     // (AUTO sends short chunks to the FP32 kernel; an explicit FDD_KERNEL_TENSOR request does not)
     if (kernel == FDD_KERNEL_TENSOR && j_begin % fdd::kSymT == 0 && !mirror &&
         rows >= (p->kernel_request == FDD_KERNEL_TENSOR ? 1 : kTensorMinRows)) {
         // fp16 operands: X times a power of two such that |X| <= 255 nsamps cannot overflow them
         int e = 0;
-        frexp((p->offset != 0.f ? 128.0 : 255.0) * (double)p->nsamps, &e);      // |X| < 2^e
+        frexp((p->padded ? 256.0 : 128.0) * (double)p->nsamps, &e);      // |X| < 2^e
         const float xscale = (float)ldexp(1.0, 15 - e);
         const int per = fdd::kTcT * (fdd::kTcRows / 2);                          // trial DMs per launch
         for (int r0 = 0; r0 < rows; r0 += per) {
@@ -604,8 +670,19 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
 // a4 with the plan's kernel; FDD_KERNEL_MIXED: runs of 32-DM tiles that are arithmetic progressions
 // take the shared-recurrence kernel, the tiles in between (a change of DM step inside them) the
 // generic one.
+int launch_rotate_sum_plain(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
+                            cudaStream_t s, bool mirror);
+
 int launch_rotate_sum(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
                       cudaStream_t s, bool mirror = false)
+{
+    const int rc = launch_rotate_sum_plain(p, j_begin, rows, dst, opitch, mode, s, mirror);
+    if (rc != FDD_OK) return rc;
+    return launch_pad_add_table(p, j_begin, rows, dst, opitch, mode, s);
+}
+
+int launch_rotate_sum_plain(fdd_plan* p, int j_begin, int rows, float2* dst, long long opitch, int mode,
+                            cudaStream_t s, bool mirror)
 {
     if (p->kernel != FDD_KERNEL_MIXED || j_begin % fdd::kSymT != 0)
         return launch_rotate_sum_kernel(p, p->kernel == FDD_KERNEL_MIXED ? FDD_KERNEL_GENERIC : p->kernel,
@@ -676,8 +753,9 @@ int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer&
     tm.begin(FDD_STAGE_R2C, 1);
     if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     if (cufftExecR2C(p->r2c, p->xreal, p->X) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    const int rcp = launch_pad_add_rect(p, p->X, s);
     tm.end();
-    return FDD_OK;
+    return rcp;
 }
 
 // Stages a4+a5 from the spectra in p->X.  chunk_done (optional) is called after each DM chunk
@@ -856,6 +934,7 @@ int fdd_plan_prepare(fdd_plan* p, int mode)
     const bool generic_rows = p->kernel == FDD_KERNEL_GENERIC || p->kernel == FDD_KERNEL_MIXED ||
                               (mode == FDD_MODE_TIME && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0);
     if (generic_rows && p->rec_pshift >= 0 && (rc = ensure_rec_tables(p, nullptr)) != FDD_OK) return rc;
+    if ((rc = ensure_pad_table(p, nullptr)) != FDD_OK) return rc;
     // launch shapes of the shared-recurrence kernel for the chunks an execute will step through
     if (p->kernel == FDD_KERNEL_SYMMETRIC2) {
         const int step = mode == FDD_MODE_TIME ? p->y_rows : p->ndm;
@@ -1022,6 +1101,112 @@ int fdd_tdd_execute(fdd_plan* p, const unsigned char* in_u8, float* out, void* c
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
+int fdd_execute_beams(fdd_plan* p, const unsigned char* in_u8, void* out, int nbeams, int mode,
+                      void* cuda_stream)
+{
+    if (check_plan(p) != FDD_OK || !in_u8 || !out || nbeams < 1 ||
+        (mode != FDD_MODE_TIME && mode != FDD_MODE_FOURIER))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok) return FDD_ERR_CUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t in_beam = (size_t)p->nsamps * p->nchans;
+    const size_t out_beam = mode == FDD_MODE_TIME ? (size_t)p->ndm * p->nsamps_out * sizeof(float)
+                                                  : (size_t)p->ndm * p->nbins_out * sizeof(float2);
+    // beams per tensor-core launch: the 64 tile rows of its Z operand are shared out between them
+    int group = 1;
+    const bool tensor = tensor_ok(p) && (p->kernel_request == FDD_KERNEL_AUTO || p->kernel_request == FDD_KERNEL_TENSOR);
+    if (tensor && nbeams > 1) group = p->ndm <= 1024 ? 4 : (p->ndm <= 2048 ? 2 : 1);
+    int rc;
+    if (group > 1 && mode == FDD_MODE_TIME) {
+        if ((rc = ensure_time_resources(p, 0)) != FDD_OK) return rc;
+        if (p->y_rows != p->ndm) group = 1;               // (Y is chunked: one beam at a time)
+    }
+    StageTimer tm(p, s);
+    if (group == 1) {
+        // no sharing possible (more than 2048 trial DMs, or not a uniform DM grid): beam after beam
+        for (int b = 0; b < nbeams; ++b) {
+            if ((rc = run_pre(p, in_u8 + (size_t)b * in_beam, s, tm)) != FDD_OK) return rc;
+            rc = run_post(p, static_cast<char*>(out) + (size_t)b * out_beam, mode, s, tm, [](int, int) {}, 0, 0,
+                          [](int) {});
+            if (rc != FDD_OK) return rc;
+        }
+        return FDD_OK;
+    }
+    if (p->beam_group < group) {
+        if (cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
+        if (p->beam_X) { cudaFree(p->beam_X); p->scratch_bytes -= (size_t)p->beam_group * p->nchans * p->xpitch * sizeof(float2); p->beam_X = nullptr; }
+        if (p->beam_Y) { cudaFree(p->beam_Y); p->scratch_bytes -= (size_t)p->beam_group * p->ndm * p->ypitch * sizeof(float2); p->beam_Y = nullptr; }
+        p->beam_group = 0;
+        if ((rc = dev_alloc(p, &p->beam_X, (size_t)group * p->nchans * p->xpitch)) != FDD_OK) return rc;
+        p->beam_group = group;
+    }
+    if (mode == FDD_MODE_TIME && !p->beam_Y &&
+        (rc = dev_alloc(p, &p->beam_Y, (size_t)p->beam_group * p->ndm * p->ypitch)) != FDD_OK)
+        return rc;
+    const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
+    const double dc_raw = p->padded ? 0.0 : (double)p->offset * (double)p->nchans * (double)p->nsamps;
+    const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
+    int e = 0;
+    frexp((p->padded ? 256.0 : 128.0) * (double)p->nsamps, &e);
+    const float xscale = (float)ldexp(1.0, 15 - e);
+    const long long xstride = (long long)p->nchans * p->xpitch;
+    for (int b0 = 0; b0 < nbeams; b0 += group) {
+        const int gb = nbeams - b0 < group ? nbeams - b0 : group;
+        const int glaunch = gb == 3 ? 0 : gb;
+        for (int b = 0; b < gb; ++b) {
+            // a2 + a3 of beam b0 + b into its slot of beam_X
+            tm.begin(FDD_STAGE_UNPACK, 1);
+            rc = launch_unpack(p, in_u8 + (size_t)(b0 + b) * in_beam, s);
+            tm.end();
+            if (rc != FDD_OK) return rc;
+            tm.begin(FDD_STAGE_R2C, 1);
+            if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+            if (cufftExecR2C(p->r2c, p->xreal, p->beam_X + (long long)b * xstride) != CUFFT_SUCCESS)
+                return FDD_ERR_CUFFT;
+            rc = launch_pad_add_rect(p, p->beam_X + (long long)b * xstride, s);
+            tm.end();
+            if (rc != FDD_OK) return rc;
+        }
+        // a4 for the whole group: one launch, the pair phasors are made once for all its beams
+        // (the kernel shares its operand rows among 1, 2 or 4 beams: a group of 3 runs as 2 + 1)
+        float2* dst = mode == FDD_MODE_TIME ? p->beam_Y
+                                            : static_cast<float2*>(out) + (size_t)b0 * p->ndm * p->nbins_out;
+        const long long opitch = mode == FDD_MODE_TIME ? p->ypitch : p->nbins_out;
+        const long long ostride = (long long)p->ndm * opitch;
+        tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+        if (glaunch == gb) {
+            rc = fdd::tc_launch(p->sym, p->nfft, p->beam_X, p->xpitch, p->nchans, p->nbins_out, p->ndm, 0, p->ndm,
+                                dst, opitch, scale, mode == FDD_MODE_TIME ? 1 : 0, dc_add, xscale, p->num_sms, s,
+                                glaunch, xstride, ostride);
+        } else {
+            rc = fdd::tc_launch(p->sym, p->nfft, p->beam_X, p->xpitch, p->nchans, p->nbins_out, p->ndm, 0, p->ndm,
+                                dst, opitch, scale, mode == FDD_MODE_TIME ? 1 : 0, dc_add, xscale, p->num_sms, s,
+                                2, xstride, ostride);
+            if (rc == 0)
+                rc = fdd::tc_launch(p->sym, p->nfft, p->beam_X + 2 * xstride, p->xpitch, p->nchans, p->nbins_out,
+                                    p->ndm, 0, p->ndm, dst + 2 * ostride, opitch, scale,
+                                    mode == FDD_MODE_TIME ? 1 : 0, dc_add, xscale, p->num_sms, s, 1, 0, 0);
+        }
+        for (int b = 0; b < gb && rc == 0; ++b)
+            rc = launch_pad_add_table(p, 0, p->ndm, dst + (long long)b * ostride, opitch, mode, s);
+        tm.end();
+        if (rc != 0) return rc == -5 ? FDD_ERR_UNSUPPORTED : (rc < 0 && rc > -5 ? rc : FDD_ERR_CUDA);
+        if (mode == FDD_MODE_TIME) {
+            for (int b = 0; b < gb; ++b) {
+                int nl = 0;
+                tm.begin(FDD_STAGE_C2R, 0);
+                rc = launch_c2r_rows(p, 0, p->ndm, p->beam_Y + (long long)b * ostride,
+                                     static_cast<float*>(out) + (size_t)(b0 + b) * p->ndm * p->nsamps_out, s, &nl);
+                tm.end();
+                p->launches[FDD_STAGE_C2R] += nl;
+                if (rc != FDD_OK) return rc;
+            }
+        }
+    }
+    return FDD_OK;
+}
+
 int fdd_tc_selftest(const void* a_f16_dev, const void* b_f16_dev, float* d_dev, void* cuda_stream)
 {
     if (!a_f16_dev || !b_f16_dev || !d_dev) return FDD_ERR_INVALID_ARG;
@@ -1093,6 +1278,13 @@ int fdd_plan_get_spectrum(const fdd_plan* p, void** x_dev, long long* pitch_elem
     *x_dev = p->X;
     *pitch_elems = p->xpitch;
     if (dc_removed) *dc_removed = (double)p->offset * (double)p->nsamps;
+    return FDD_OK;
+}
+
+int fdd_plan_get_padding(const fdd_plan* p, long long* exact_bins)
+{
+    if (!p || !exact_bins) return FDD_ERR_INVALID_ARG;
+    *exact_bins = p->padded ? p->pad_k : 0;
     return FDD_OK;
 }
 

@@ -37,12 +37,15 @@ k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int 
             const int tr = trow + 16 * i;
             const long long t = t0 + tr;
             uchar4 v = make_uchar4(0, 0, 0, 0);
-            if (t < nsamps && c0 + cq < nchans)
+            float off = 0.f;                     // the padding is zero, not -offset
+            if (t < nsamps && c0 + cq < nchans) {
                 v = *reinterpret_cast<const uchar4*>(in + t * nchans + c0 + cq);
-            tile[cq + 0][tr] = (float)v.x - offset;
-            tile[cq + 1][tr] = (float)v.y - offset;
-            tile[cq + 2][tr] = (float)v.z - offset;
-            tile[cq + 3][tr] = (float)v.w - offset;
+                off = offset;
+            }
+            tile[cq + 0][tr] = (float)v.x - off;
+            tile[cq + 1][tr] = (float)v.y - off;
+            tile[cq + 2][tr] = (float)v.z - off;
+            tile[cq + 3][tr] = (float)v.w - off;
         }
     } else {
         const int trow = tid >> 6;          // 0..3

@@ -71,7 +71,7 @@ def test_unpack_and_r2c_against_fp64_rfft(F, nchans, nsamps):
         plan.execute(d_in, out, F.FDD_MODE_TIME)
         torch.cuda.synchronize()
         ptr, pitch, dc_removed = plan.get_spectrum()
-        assert dc_removed == (128.0 * nsamps if nsamps == plan.nfft else 0.0)
+        assert dc_removed == 128.0 * nsamps
         assert plan.nfft == O.next_pow2(nsamps) and plan.nbins == plan.nfft // 2 + 1
         # view the plan's X in place through the CUDA array interface
         class _View:
@@ -82,6 +82,11 @@ def test_unpack_and_r2c_against_fp64_rfft(F, nchans, nsamps):
         X = (X[..., 0] + 1j * X[..., 1])[:, :plan.nbins]
         X[:, 0] += dc_removed                      # the mean a2 takes out of the fp32 FFT
         ref = np.fft.rfft(O.unpack(u8, plan.nfft), axis=-1)
+        kx = plan.get_padding()                    # zero padded: the mean is a rectangle, whose spectrum
+        assert kx == (0 if nsamps == plan.nfft else min(plan.nbins, 4096))   # is missing below bin kx
+        if kx:
+            rect = np.zeros(plan.nfft); rect[:nsamps] = 128.0
+            ref[:, 1:kx] -= np.fft.rfft(rect)[1:kx]
         # fp32 FFT of u8 data: error relative to the rms of the non-DC bins
         rms = np.sqrt((np.abs(ref[:, 1:]) ** 2).mean())
         assert np.abs(X - ref)[:, 1:].max() <= 2e-5 * rms * np.sqrt(np.log2(plan.nfft))
@@ -690,3 +695,61 @@ def test_tensor_core_kernel_against_the_oracle(F, oracle_c, nchans, nsamps, ndm,
         got = _run(F, plan, u8, mode)[rows]
     worst = parity.assert_rows(got, ref, mode, f"tensor {nchans}x{nsamps}x{ndm}/{mode}")
     print("tensor", nchans, nsamps, ndm, mode, worst)
+
+
+# ------------------------------------------------------------------ row f1: several beams, one plan
+@pytest.mark.parametrize("mode", ["time", "fourier"])
+@pytest.mark.parametrize("nbeams,ndm,kernel", [
+    (1, 96, "auto"),        # one beam = fdd_execute
+    (4, 200, "auto"),       # one group of 4 beams sharing the pair phasors (tensor-core launch)
+    (7, 1000, "auto"),      # 4 + 3 beams (the group of 3 runs as 2 + 1)
+    (3, 1500, "auto"),      # 1025..2048 trial DMs: groups of 2
+    (2, 70, "generic"),     # a plan that cannot share: beam after beam
+])
+def test_multi_beam_against_the_oracle(F, oracle_c, nbeams, ndm, kernel, mode):
+    """fdd_execute_beams: every beam against the oracle's beam-by-beam definition."""
+    import torch
+    nchans, nsamps = 96, 2048
+    ws = [synth.small_workload(900 + 7 * b, nchans, nsamps, ndm, dm_step=0.07, mode=mode) for b in range(nbeams)]
+    beams = np.stack([synth.make_filterbank(w) for w in ws])
+    d = _delays_for(ws[0])
+    rows = list(range(ndm)) if ndm <= 200 else sorted(set(range(0, ndm, 97)) | {63, 64, ndm - 1})
+    ref = O.fdd_beams(beams, d, rows, mode=mode)
+    with _plan_for(F, ws[0]) as plan:
+        _set_kernel(F, plan, kernel)
+        shape = (nbeams, ndm, plan.nsamps) if mode == "time" else (nbeams, ndm, plan.nbins, 2)
+        out = torch.full(shape, float("nan"), dtype=torch.float32, device="cuda")
+        plan.execute_beams(torch.from_numpy(beams).cuda(), out, nbeams,
+                           F.FDD_MODE_TIME if mode == "time" else F.FDD_MODE_FOURIER)
+        torch.cuda.synchronize()
+        got = out[:, rows].cpu().numpy()
+        if mode == "fourier":
+            got = got[..., 0] + 1j * got[..., 1]
+    for b in range(nbeams):
+        parity.assert_rows(got[b], ref[b], mode, f"beam {b} of {nbeams}/{ndm}/{mode}")
+
+
+@pytest.mark.slow
+def test_multi_beam_config3_eight_beams(F, oracle_c):
+    """BASELINE.json config 3 (1024 channels x 2^20 samples x 1024 trial DMs) with 8 beams: beam 0 is
+    the config-3 input, the others fresh seeded noise; two tensor-core launches of 4 beams each."""
+    import torch
+    w = synth.workload("config3")
+    _, u8 = _FullSize.input("config3")
+    nbeams = 8
+    torch.cuda.empty_cache()
+    d_in = torch.empty((nbeams, w.nsamps, w.nchans), dtype=torch.uint8, device="cuda")
+    d_in[0] = torch.from_numpy(u8).cuda()
+    gen = torch.Generator(device="cuda").manual_seed(4242)
+    for b in range(1, nbeams):
+        d_in[b] = (torch.randn((w.nsamps, w.nchans), generator=gen, device="cuda") * 16 + 128).round().clamp(0, 255).to(torch.uint8)
+    check = {0: [0, 37, 527, 1023], 5: [1, 300, 1023]}
+    with _plan_for(F, w) as plan:
+        out = torch.empty((nbeams, w.ndm, w.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute_beams(d_in, out, nbeams, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        for b, rows in check.items():
+            beam = d_in[b].cpu().numpy()
+            ref = O.fdd_rows(beam, _delays_for(w), rows, mode="time")
+            worst = parity.assert_rows(out[b, rows].cpu().numpy(), ref, "time", f"config 3, beam {b} of 8")
+            print("config3 beams", b, rows, worst)

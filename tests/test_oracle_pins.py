@@ -318,3 +318,25 @@ def test_generator_is_deterministic_and_shaped():
     assert synth.workload("sweep", ndm=128).ndm == 128
     assert synth.workload("config5").mode == "fourier"
     assert abs(max(synth.workload("config5").dm_list) - 81.91) < 1e-9
+
+
+# ---------------------------------------------------------------- row f1: beams
+def test_beams_are_independent_and_linear(oracle_c):
+    """fdd_beams adds no arithmetic: beam b equals the single-beam result; identical beams give
+    identical rows; a beam at DM 0 is its own channel sum (P2 per beam); and, Eq. 7 being linear in
+    the data, the spectrum of the sample-wise sum of two beams is the sum of their
+    spectra - checked on inputs small enough that the sum stays in 8 bits."""
+    rng = np.random.default_rng(71)
+    beams = rng.integers(0, 120, (3, 512, 6), dtype=np.uint8)
+    beams[2] = beams[0]
+    d = O.delay_table(6, 1200.0, 1500.0, 64e-6, [0.0, 3.7, 11.0, 40.0])
+    Y = O.fdd_beams(beams, d, mode="fourier")
+    y = O.fdd_beams(beams, d, mode="time")
+    assert Y.shape == (3, 4, 257) and y.shape == (3, 4, 512)
+    for b in range(3):
+        assert np.abs(y[b] - O.fdd_fft(beams[b], d)).max() <= 1e-11 * np.abs(y[b]).max()
+        assert np.abs(y[b][0] - beams[b].astype(np.int64).sum(axis=1)).max() <= 1e-9
+    assert np.array_equal(y[0], y[2]) and not np.array_equal(y[0], y[1])
+    both = (beams[0].astype(np.int64) + beams[1]).astype(np.uint8)
+    Ysum = O.fdd_fft(both, d, mode="fourier")
+    assert np.abs(Ysum - (Y[0] + Y[1])).max() <= 1e-10 * np.abs(Ysum).max()
