@@ -67,6 +67,8 @@ def parse_args():
     ap.add_argument("--beams", type=int, default=1, metavar="B",
                     help="row f1: B beams per step through fdd_execute_beams (beam 0 = the workload's "
                          "input, the others seeded noise made on the device); the rate counts all beams")
+    ap.add_argument("--inverse", default="cufft", choices=["cufft", "two_pass"],
+                    help="step a5: cuFFT (default) or the hand-written two-pass inverse")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -313,6 +315,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
     if args.decimate:
         plan.set_decimation(args.decimate)
+    if args.inverse == "two_pass":
+        plan.set_inverse(F.FDD_INVERSE_TWO_PASS)
     ns_out, nbins = plan.output_shape()                   # = (nsamps, nbins) at full rate
     nfft_out = nfft >> args.decimate
     d_in = torch.from_numpy(u8).cuda()

@@ -84,6 +84,18 @@ enum fdd_kernel {
                                   operands and fp32 accumulation in TMEM           */
 };
 
+/* Step a5 (fdd_plan_set_inverse). */
+enum fdd_inverse {
+    FDD_INVERSE_CUFFT = 0,     /* cuFFT (C2R, or the half-length C2C fed by SYMMETRIC2's fused pre-twiddle):
+                                  the default - at 2^20 points it runs at 70 % of the HBM roofline of a
+                                  two-pass transform                                                  */
+    FDD_INVERSE_TWO_PASS = 1   /* the hand-written two-pass inverse real transform, nfft = 2^7 .. 2^23: forms
+                                  the half-length spectrum in its first pass and adds the series' mean
+                                  after the transform, so fp32 works on a series of rms sigma instead of
+                                  256 sigma (TIME-mode error about 2x smaller); at present 2.7x slower
+                                  than cuFFT, cuFFT for other lengths                      */
+};
+
 /* Stage indices for fdd_plan_get_stage_ms. */
 enum fdd_stage {
     FDD_STAGE_UNPACK = 0, FDD_STAGE_R2C = 1, FDD_STAGE_ROTATE_SUM = 2, FDD_STAGE_C2R = 3,
@@ -150,6 +162,10 @@ int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
  * does the same work inside its first execute.  (The staging buffers of fdd_execute_host and the
  * tables of fdd_tdd_execute are still made on their first call.) */
 int fdd_plan_prepare(fdd_plan *plan, int mode);
+
+/* Choose the inverse transform of step a5 (enum fdd_inverse; default FDD_INVERSE_CUFFT).  Synchronises the device and drops the
+ * TIME-mode scratch (re-made by fdd_plan_prepare or the next TIME execute). */
+int fdd_plan_set_inverse(fdd_plan *plan, int which);
 
 /* TIME mode keeps the sums Y of a chunk of trial DMs in plan-owned scratch between a4 and a5.  The
  * chunk is as many rows as fit `bytes` (default 24 GiB, and never more than half of the free

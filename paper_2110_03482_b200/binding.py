@@ -17,6 +17,7 @@ FDD_MODE_TIME, FDD_MODE_FOURIER = 0, 1
 FDD_KERNEL_AUTO, FDD_KERNEL_GENERIC, FDD_KERNEL_SYMMETRIC, FDD_KERNEL_SYMMETRIC2 = 0, 1, 2, 3
 FDD_KERNEL_MIXED = 4
 FDD_KERNEL_TENSOR = 5
+FDD_INVERSE_CUFFT, FDD_INVERSE_TWO_PASS = 0, 1
 FDD_OK = 0
 FDD_NUM_STAGES = 6
 STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift_add")
@@ -24,7 +25,7 @@ STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift
 EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
     "fdd_plan_set_decimation", "fdd_plan_get_output_shape", "fdd_plan_prepare",
-    "fdd_plan_set_y_budget",
+    "fdd_plan_set_y_budget", "fdd_plan_set_inverse",
     "fdd_execute", "fdd_execute_host", "fdd_execute_beams", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_plan_get_padding", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
@@ -69,6 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_set_decimation.argtypes = [vp, c_int]
     lib.fdd_plan_prepare.argtypes = [vp, c_int]
     lib.fdd_plan_set_y_budget.argtypes = [vp, ctypes.c_size_t]
+    lib.fdd_plan_set_inverse.argtypes = [vp, c_int]
     lib.fdd_plan_get_output_shape.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong),
                                               ctypes.POINTER(ctypes.c_longlong)]
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
@@ -207,6 +209,10 @@ class Plan:
     def prepare(self, mode: int = FDD_MODE_TIME) -> None:
         """Do every lazy allocation / upload of ``mode`` now, so execute never synchronises."""
         _check(load_library().fdd_plan_prepare(self._h, int(mode)), "fdd_plan_prepare")
+
+    def set_inverse(self, which: int) -> None:
+        """FDD_INVERSE_CUFFT (default) or FDD_INVERSE_TWO_PASS (hand-written, keeps the mean out of fp32)."""
+        _check(load_library().fdd_plan_set_inverse(self._h, int(which)), "fdd_plan_set_inverse")
 
     def set_y_budget(self, nbytes: int) -> None:
         """Cap the TIME-mode Y scratch (trial DMs are then processed in chunks); 0 = default."""

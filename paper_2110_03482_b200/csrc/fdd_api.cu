@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "fdd_kernels_generic.cuh"
+#include "fdd_kernels_ifft.cuh"
 #include "fdd_kernels_krec.cuh"
 #include "fdd_kernels_pad.cuh"
 #include "fdd_kernels_pre.cuh"
@@ -32,6 +33,7 @@ constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per
 constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
 constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
+constexpr int kIfftBatch = 16;                        // rows per pass of the own inverse (ring: 2 x 64 MiB at 2^20)
 constexpr int kTensorMinRows = 1024;                  // launches with fewer trial DMs take the FP32 kernels
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
@@ -99,6 +101,12 @@ struct fdd_plan {
     int c2r_batch = 0, c2r_tail_batch = 0;
     void* fft_ws = nullptr;
     size_t fft_ws_bytes = 0;
+    // a5 by the hand-written two-pass transform (fdd_kernels_ifft.cuh) instead of cuFFT
+    int inverse_request = FDD_INVERSE_CUFFT;
+    bool ifft_on = false;                // decided with the TIME-mode resources
+    bool dc_in_bin0 = true;              // a4 restores the mean in bin 0 (false: the own inverse adds it)
+    float2* ifft_ring = nullptr;         // [2][kIfftBatch][nfft_out / 2]
+    size_t ifft_ring_bytes = 0;
     // multi-beam execution (fdd_execute_beams): spectra and TIME-mode sums of one group of beams
     float2* beam_X = nullptr;            // [beam_group][nchans][xpitch]
     float2* beam_Y = nullptr;            // [beam_group][ndm][ypitch]
@@ -326,7 +334,10 @@ int make_c2r_plan(fdd_plan* p, int family, cufftHandle* h, int batch, size_t* ws
 // spectrum the mirrored sym2 epilogue writes, 0 = cuFFT's C2R from Y.
 int time_family(const fdd_plan* p)
 {
-    // (a zero-padded plan adds the rectangle's table to Y after a4, so a4 must write plain sums)
+    // (a zero-padded plan adds the rectangle's table to Y after a4, so a4 must write plain sums; the
+    //  hand-written inverse forms the half-length spectrum itself)
+    int m1, m2;
+    if (p->inverse_request == FDD_INVERSE_TWO_PASS && fdd::ifft_split(p->nfft_out, &m1, &m2)) return 0;
     return (p->kernel == FDD_KERNEL_SYMMETRIC2 && p->nfft_out >= 4 && !p->padded) ? 1 : 0;
 }
 
@@ -417,6 +428,13 @@ void drop_time_resources(fdd_plan* p)
         p->scratch_bytes -= (size_t)p->beam_group * p->ndm * p->ypitch * sizeof(float2);
         p->beam_Y = nullptr;
     }
+    if (p->ifft_ring) {
+        cudaFree(p->ifft_ring);
+        p->scratch_bytes -= p->ifft_ring_bytes;
+        p->ifft_ring = nullptr;
+        p->ifft_ring_bytes = 0;
+    }
+    p->ifft_on = false;
     p->y_rows = 0;
     p->c2r_tail_batch = 0;
     p->sym2_shapes.clear();
@@ -434,6 +452,13 @@ int ensure_time_family(fdd_plan* p, int* family_out)
         if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
     }
     *family_out = family;
+    int m1, m2;
+    p->ifft_on = family == 0 && p->inverse_request == FDD_INVERSE_TWO_PASS && fdd::ifft_split(p->nfft_out, &m1, &m2);
+    if (p->ifft_on && !p->ifft_ring) {
+        const size_t n = (size_t)2 * kIfftBatch * (size_t)(p->nfft_out / 2);
+        if ((rc = dev_alloc(p, &p->ifft_ring, n)) != FDD_OK) return rc;
+        p->ifft_ring_bytes = n * sizeof(float2);
+    }
     return FDD_OK;
 }
 
@@ -459,6 +484,7 @@ void destroy_plan(fdd_plan* p)
     cudaFree(p->stage_in);
     cudaFree(p->stage_out);
     cudaFree(p->pad_tab);
+    cudaFree(p->ifft_ring);
     cudaFree(p->beam_X);
     cudaFree(p->beam_Y);
     fdd::sym_free_tables(&p->sym);
@@ -609,7 +635,8 @@ int launch_rotate_sum_kernel(fdd_plan* p, int kernel, int j_begin, int rows, flo
     const int real_edges = mode == FDD_MODE_TIME ? 1 : 0;      // reading S8
     // bin 0 of every trial DM gets back the mean a2 removed: offset * nchans * nsamps (* scale)
     const double dc_raw = p->padded ? 0.0 : (double)p->offset * (double)p->nchans * (double)p->nsamps;
-    const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
+    const bool dc_in_bin0 = p->dc_in_bin0;
+    const float dc_add = mode == FDD_MODE_TIME ? (dc_in_bin0 ? (float)(dc_raw / (double)p->nfft) : 0.f) : (float)dc_raw;
     // (AUTO sends short chunks to the FP32 kernel; an explicit FDD_KERNEL_TENSOR request does not)
     if (kernel == FDD_KERNEL_TENSOR && j_begin % fdd::kSymT == 0 && !mirror &&
         rows >= (p->kernel_request == FDD_KERNEL_TENSOR ? 1 : kTensorMinRows)) {
@@ -707,6 +734,15 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
                     int* launches)
 {
     // ysrc: [rows][ypitch]; dst: caller rows (pitch nsamps).
+    if (p->ifft_on && family == 0) {
+        // the mean a2 removed comes back here, after the transform (not zero padded: a constant)
+        const float mean = p->padded ? 0.f
+                                     : (float)((double)p->offset * (double)p->nchans * (double)p->nsamps / (double)p->nfft);
+        const int rc = fdd::ifft_launch(ysrc, p->ypitch, rows, dst, p->nsamps_out, p->nsamps_out, p->nfft_out, mean,
+                                        p->ifft_ring, kIfftBatch, s);
+        *launches += 2 * ((rows + kIfftBatch - 1) / kIfftBatch);
+        return rc == 0 ? FDD_OK : (rc == -5 ? FDD_ERR_UNSUPPORTED : FDD_ERR_CUDA);
+    }
     const bool direct = (p->nsamps_out == p->nfft_out);
     int done = 0;
     while (done < rows) {
@@ -792,7 +828,9 @@ int run_post(fdd_plan* p, void* out, int mode, cudaStream_t s, StageTimer& tm, F
         const int rows = (p->ndm - j0 < step) ? p->ndm - j0 : step;
         chunk_begin(j0);
         tm.begin(FDD_STAGE_ROTATE_SUM, 1);
+        p->dc_in_bin0 = !p->ifft_on;
         rc = launch_rotate_sum(p, j0, rows, p->Y, p->ypitch, mode, s, family == 1);
+        p->dc_in_bin0 = true;
         tm.end();
         if (rc != FDD_OK) return rc;
         int nl = 0;
@@ -908,6 +946,17 @@ int fdd_plan_set_kernel(fdd_plan* p, int kernel)
     if (kernel == FDD_KERNEL_SYMMETRIC2 && !p->sym_ok) return FDD_ERR_UNSUPPORTED;
     p->kernel_request = kernel;
     p->kernel = resolve_kernel(p, kernel);
+    return FDD_OK;
+}
+
+int fdd_plan_set_inverse(fdd_plan* p, int which)
+{
+    if (check_plan(p) != FDD_OK || (which != FDD_INVERSE_TWO_PASS && which != FDD_INVERSE_CUFFT))
+        return FDD_ERR_INVALID_ARG;
+    DeviceGuard g(p->device);
+    if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
+    drop_time_resources(p);
+    p->inverse_request = which;
     return FDD_OK;
 }
 
@@ -1118,6 +1167,7 @@ int fdd_execute_beams(fdd_plan* p, const unsigned char* in_u8, void* out, int nb
     const bool tensor = tensor_ok(p) && (p->kernel_request == FDD_KERNEL_AUTO || p->kernel_request == FDD_KERNEL_TENSOR);
     if (tensor && nbeams > 1) group = p->ndm <= 1024 ? 4 : (p->ndm <= 2048 ? 2 : 1);
     int rc;
+    int family = 0;
     if (group > 1 && mode == FDD_MODE_TIME) {
         if ((rc = ensure_time_resources(p, 0)) != FDD_OK) return rc;
         if (p->y_rows != p->ndm) group = 1;               // (Y is chunked: one beam at a time)
@@ -1146,7 +1196,8 @@ int fdd_execute_beams(fdd_plan* p, const unsigned char* in_u8, void* out, int nb
         return rc;
     const float scale = mode == FDD_MODE_TIME ? (float)(1.0 / (double)p->nfft) : 1.0f;
     const double dc_raw = p->padded ? 0.0 : (double)p->offset * (double)p->nchans * (double)p->nsamps;
-    const float dc_add = (float)(mode == FDD_MODE_TIME ? dc_raw / (double)p->nfft : dc_raw);
+    if (mode == FDD_MODE_TIME && (rc = ensure_time_family(p, &family)) != FDD_OK) return rc;
+    const float dc_add = mode == FDD_MODE_TIME ? (p->ifft_on ? 0.f : (float)(dc_raw / (double)p->nfft)) : (float)dc_raw;
     int e = 0;
     frexp((p->padded ? 256.0 : 128.0) * (double)p->nsamps, &e);
     const float xscale = (float)ldexp(1.0, 15 - e);

@@ -753,3 +753,29 @@ def test_multi_beam_config3_eight_beams(F, oracle_c):
             ref = O.fdd_rows(beam, _delays_for(w), rows, mode="time")
             worst = parity.assert_rows(out[b, rows].cpu().numpy(), ref, "time", f"config 3, beam {b} of 8")
             print("config3 beams", b, rows, worst)
+
+
+# ------------------------------------------------------------------ step a5: both inverse transforms
+@pytest.mark.parametrize("kernel", ["auto", "symmetric", "tensor"])
+@pytest.mark.parametrize("nchans,nsamps,ndm,step", [
+    (64, 8192, 40, 1.5),             # nfft 2^13: M = 4096 = 64 x 64
+    (33, 128, 5, 0.4),               # the shortest series the hand-written inverse takes (M = 8 x 8)
+    (20, 6000, 70, 0.9),             # zero padded, output cropped to 6000 of 8192 samples
+    (8, 1 << 17, 33, 2.0),           # M = 2^16 = 256 x 256
+    (12, 1001, 9, 0.3),              # odd series length
+])
+def test_inverse_transform_choices(F, oracle_c, nchans, nsamps, ndm, step, kernel):
+    """FDD_INVERSE_TWO_PASS (the hand-written two-pass inverse, which also restores the mean after the
+    transform) and FDD_INVERSE_CUFFT (C2R, or SYMMETRIC2's fused pre-twiddle + C2C) against the oracle."""
+    w = synth.small_workload(1300 + nchans, nchans, nsamps, ndm, dm_step=step)
+    u8 = synth.make_filterbank(w)
+    ref = O.fdd_rows(u8, _delays_for(w), range(ndm), mode="time")
+    with _plan_for(F, w) as plan:
+        _set_kernel(F, plan, kernel)
+        for which in (F.FDD_INVERSE_TWO_PASS, F.FDD_INVERSE_CUFFT, F.FDD_INVERSE_TWO_PASS):
+            plan.set_inverse(which)
+            got = _run(F, plan, u8, "time")
+            worst = parity.assert_rows(got, ref, "time", f"inverse {which}/{kernel}/{nchans}x{nsamps}")
+            print("inverse", which, kernel, nchans, nsamps, worst)
+        with pytest.raises(F.FddError):
+            plan.set_inverse(7)
