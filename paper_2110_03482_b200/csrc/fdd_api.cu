@@ -117,6 +117,7 @@ struct fdd_plan {
     size_t stage_out_bytes = 0;
     cudaStream_t copy_stream = nullptr;
     std::vector<cudaEvent_t> chunk_events;
+    std::vector<cudaEvent_t> in_events;
     // profiling
     bool profiling = false;
     std::vector<StageEvent> events;
@@ -490,6 +491,7 @@ void destroy_plan(fdd_plan* p)
     fdd::sym_free_tables(&p->sym);
     for (auto& e : p->events) { cudaEventDestroy(e.beg); cudaEventDestroy(e.end); }
     for (auto& e : p->chunk_events) cudaEventDestroy(e);
+    for (auto& e : p->in_events) cudaEventDestroy(e);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     cudaGetLastError();
     delete p;
@@ -567,18 +569,21 @@ struct StageTimer {
     }
 };
 
-int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s)
+// time tiles [tile0, tile0 + ntiles) of 64 samples (ntiles < 0: all of them)
+int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, long long tile0 = 0,
+                  long long ntiles = -1)
 {
-    dim3 grid((unsigned)((p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile),
-              (unsigned)((p->nchans + fdd::kUnpackTile - 1) / fdd::kUnpackTile));
+    if (ntiles < 0) ntiles = (p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile;
+    if (ntiles == 0) return FDD_OK;
+    dim3 grid((unsigned)ntiles, (unsigned)((p->nchans + fdd::kUnpackTile - 1) / fdd::kUnpackTile));
     float* xf = p->xreal;
     const bool vec = (p->nchans % 4 == 0) && ((uintptr_t)in_u8 % 4 == 0);
     if (vec)
         fdd::k_unpack_transpose<4><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        p->nfft, p->offset);
+                                                        p->nfft, p->offset, tile0);
     else
         fdd::k_unpack_transpose<1><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        p->nfft, p->offset);
+                                                        p->nfft, p->offset, tile0);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
@@ -780,11 +785,14 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
 int check_plan(const fdd_plan* p) { return p ? FDD_OK : FDD_ERR_INVALID_ARG; }
 
 // Stages a2+a3.
-int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer& tm)
+int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer& tm, bool unpacked = false)
 {
-    tm.begin(FDD_STAGE_UNPACK, 1);
-    int rc = launch_unpack(p, in_u8, s);
-    tm.end();
+    int rc = FDD_OK;
+    if (!unpacked) {
+        tm.begin(FDD_STAGE_UNPACK, 1);
+        rc = launch_unpack(p, in_u8, s);
+        tm.end();
+    }
     if (rc != FDD_OK) return rc;
     tm.begin(FDD_STAGE_R2C, 1);
     if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
@@ -1058,10 +1066,40 @@ int fdd_execute_host(fdd_plan* p, const unsigned char* in_host, void* out_host, 
     if (!p->copy_stream &&
         cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess)
         return FDD_ERR_CUDA;
-    if (cudaMemcpyAsync(p->stage_in, in_host, in_bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
-        return FDD_ERR_CUDA;
+    // Algorithm 1 lines 9-17: the input goes up in time blocks on the copy stream and every block is
+    // unpacked as soon as it has landed (a2 is local in time; only the R2C needs whole rows)
     StageTimer tm(p, s);
-    rc = run_pre(p, p->stage_in, s, tm);
+    {
+        constexpr int kInBlocks = 8;
+        while (p->in_events.size() < (size_t)kInBlocks) {
+            cudaEvent_t e;
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return FDD_ERR_CUDA; }
+            p->in_events.push_back(e);
+        }
+        const long long data_tiles = (p->nsamps + fdd::kUnpackTile - 1) / fdd::kUnpackTile;
+        const long long all_tiles = (p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile;
+        // (the copy stream must not run ahead of work still queued on s from an earlier call)
+        cudaEvent_t start = p->in_events[0];
+        if (cudaEventRecord(start, s) != cudaSuccess || cudaStreamWaitEvent(p->copy_stream, start, 0) != cudaSuccess)
+            return FDD_ERR_CUDA;
+        tm.begin(FDD_STAGE_UNPACK, kInBlocks);
+        for (int b = 0; b < kInBlocks; ++b) {
+            const long long tl = data_tiles * b / kInBlocks, th = b + 1 < kInBlocks ? data_tiles * (b + 1) / kInBlocks : all_tiles;
+            const long long t_lo = tl * fdd::kUnpackTile;
+            long long t_hi = th * fdd::kUnpackTile;
+            if (t_hi > p->nsamps) t_hi = p->nsamps;
+            if (t_hi > t_lo &&
+                cudaMemcpyAsync(p->stage_in + (size_t)t_lo * p->nchans, in_host + (size_t)t_lo * p->nchans,
+                                (size_t)(t_hi - t_lo) * p->nchans, cudaMemcpyHostToDevice, p->copy_stream) != cudaSuccess)
+                return FDD_ERR_CUDA;
+            if (cudaEventRecord(p->in_events[b], p->copy_stream) != cudaSuccess ||
+                cudaStreamWaitEvent(s, p->in_events[b], 0) != cudaSuccess)
+                return FDD_ERR_CUDA;
+            if ((rc = launch_unpack(p, p->stage_in, s, tl, th - tl)) != FDD_OK) return rc;
+        }
+        tm.end();
+    }
+    rc = run_pre(p, p->stage_in, s, tm, true);
     if (rc != FDD_OK) return rc;
     // two events per chunk: [2i] results ready (on s), [2i+1] copied back (on copy_stream)
     const int nchunks = (p->ndm + chunk - 1) / chunk;

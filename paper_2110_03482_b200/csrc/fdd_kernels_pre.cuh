@@ -22,11 +22,11 @@ constexpr int kUnpackTile = 64;
 template <int VEC>
 __global__ void __launch_bounds__(256)
 k_unpack_transpose(const uint8_t* __restrict__ in, float* __restrict__ out, int nchans,
-                   long long nsamps, long long nfft, long long rpitch, float offset)
+                   long long nsamps, long long nfft, long long rpitch, float offset, long long tile0)
 {
     __shared__ float tile[kUnpackTile][kUnpackTile + 1];
     const int tid = threadIdx.x;
-    const long long t0 = (long long)blockIdx.x * kUnpackTile;
+    const long long t0 = ((long long)blockIdx.x + tile0) * kUnpackTile;   // (tile0: time block of a host-streamed input)
     const int c0 = blockIdx.y * kUnpackTile;
 
     if (VEC == 4) {

@@ -500,7 +500,7 @@ class _FullSize:
         return np.stack([cls.Y[(key, j)] for j in rows])
 
 
-def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None):
+def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None, inverse="cufft"):
     """One full-size TIME execute at `ndm` trial DMs; sampled rows against the oracle."""
     import torch
     w = synth.workload(name, ndm=ndm)
@@ -515,6 +515,8 @@ def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None):
         assert plan.get_info()[5] == kernel_want
         if decimate:
             plan.set_decimation(decimate)
+        if inverse == "two_pass":
+            plan.set_inverse(F.FDD_INVERSE_TWO_PASS)
         ns_out, _ = plan.output_shape()
         d_in = torch.from_numpy(u8).cuda()
         out = torch.empty((plan.ndm, ns_out), dtype=torch.float32, device="cuda")
@@ -564,11 +566,16 @@ def test_full_size_config4_fp32_kernel(F, oracle_c, ndm):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("m", [1, 2, 3])
-def test_full_size_config4_decimated(F, oracle_c, m):
-    """Row f3 at config-4 size (512 trial DMs): reduced-length inverse transform."""
+@pytest.mark.parametrize("m,inverse", [(1, "cufft"), (2, "cufft"), (3, "cufft"), (3, "two_pass")])
+def test_full_size_config4_decimated(F, oracle_c, m, inverse):
+    """Row f3 at config-4 size (512 trial DMs): reduced-length inverse transform.  The
+    low-pass shrinks the rms of the series while cuFFT's fp32 error stays relative to its mean, so
+    m = 3 passes with little margin; the hand-written inverse (mean added after the transform) does
+    not have that dependence."""
     rows = sorted({j for j in _SWEEP_POOL if j < 512} | {511, 271, 272})
-    _full_size_point(F, "config4", 512, rows, F.FDD_KERNEL_SYMMETRIC2, decimate=m)
+    worst = _full_size_point(F, "config4", 512, rows, F.FDD_KERNEL_SYMMETRIC2, decimate=m, inverse=inverse)
+    if inverse == "two_pass":
+        assert worst["rel_l2"] <= 5e-5
 
 
 @pytest.mark.slow
