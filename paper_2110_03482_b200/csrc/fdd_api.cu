@@ -448,6 +448,15 @@ int ensure_time_family(fdd_plan* p, int* family_out)
     int family = time_family(p);
     int rc = ensure_time_resources(p, family);
     if (rc != FDD_OK) return rc;
+    if (p->kernel == FDD_KERNEL_TENSOR && p->kernel_request == FDD_KERNEL_AUTO && p->y_rows < p->ndm &&
+        p->y_rows < kTensorMinRows) {
+        // The sums of all trial DMs do not fit the Y scratch and a chunk is shorter than the tensor-core
+        // kernel pays for (its cost does not depend on the rows of a launch): this plan stays on the
+        // FP32 kernel, whose cost is proportional to the rows (the paper's 2^23-point series at 4096 DMs).
+        p->kernel = FDD_KERNEL_SYMMETRIC2;
+        family = time_family(p);
+        if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
+    }
     if (family == 1 && p->y_rows < p->ndm && p->y_rows % fdd::kSymT != 0) {
         family = 0;                          // chunks off the 32-DM tiling run the generic kernel
         if ((rc = ensure_time_resources(p, family)) != FDD_OK) return rc;
