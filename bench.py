@@ -262,13 +262,17 @@ def run_reference(args, rank: int, world: int):
 
 
 def kernel_source_hash() -> str:
-    """sha256 (first 16 hex) over the CUDA sources: ties static profile numbers to a source state."""
+    """sha256 (first 16 hex) over the CUDA sources without // comments and blank lines: ties static
+    profile numbers to a source state."""
     import glob
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_2110_03482_b200", "csrc")
     for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh"))):
         h.update(os.path.basename(f).encode())
-        h.update(open(f, "rb").read())
+        for ln in open(f, "r", errors="replace"):              # code only: comments do not stale a profile
+            code = ln.split("//", 1)[0].strip()
+            if code:
+                h.update(code.encode())
     return h.hexdigest()[:16]
 
 
