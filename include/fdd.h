@@ -142,8 +142,12 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
 
 /* Choose the a4 kernel (enum fdd_kernel).  FDD_ERR_UNSUPPORTED if FDD_KERNEL_SYMMETRIC is asked
  * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
- * 32-DM tile (tiles count from the first trial DM).  AUTO takes the fastest kernel the table
- * allows: SYMMETRIC2 (uniform DM grids, and piecewise-uniform DM plans whose segments are multiples
+ * 32-DM tile (tiles count from the first trial DM), or if FDD_KERNEL_TENSOR is asked for a table that
+ * is not ONE progression over all trial DMs (or has more than 1024 channels, or nfft > 2^23).  AUTO
+ * takes the fastest kernel the table allows: TENSOR (uniform DM grids with at least 1024 trial DMs -
+ * its cost does not depend on the number of trial DMs of a launch, up to 4096; a TIME-mode plan whose
+ * sums must be processed in chunks of fewer than 1024 rows stays on SYMMETRIC2), else
+ * SYMMETRIC2 (uniform DM grids, and piecewise-uniform DM plans whose segments are multiples
  * of 32 trial DMs), MIXED (piecewise-uniform plans with any segment lengths: only the tiles that
  * contain a step change run on the about 3.5 times slower generic kernel; at least half of the
  * tiles must be progressions), else GENERIC.  FDD_KERNEL_MIXED may be asked for whenever at least
@@ -155,8 +159,9 @@ int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
  * synchronises (it can then be captured in a CUDA graph):
  *   TIME     the Y scratch (up to 24 GiB, see fdd_plan_set_y_budget), the inverse cuFFT plans and
  *            the shared cuFFT workspace
- *   both     the bin-recurrence tables if any trial DM runs on FDD_KERNEL_GENERIC, and the launch
- *            shapes (DM-tile groups) of the shared-recurrence kernel
+ *   both     the bin-recurrence tables if any trial DM runs on FDD_KERNEL_GENERIC, the launch
+ *            shapes (DM-tile groups) of the shared-recurrence kernel, and the fp64 table of a
+ *            zero-padded plan (fdd_plan_get_spectrum)
  * Call it again after fdd_plan_set_kernel, fdd_plan_set_kdm, fdd_plan_set_decimation or
  * fdd_plan_set_y_budget.  Synchronises the device.  Not needed for correctness: an unprepared plan
  * does the same work inside its first execute.  (The staging buffers of fdd_execute_host and the

@@ -70,6 +70,7 @@ struct fdd_plan {
     // device buffers
     float2* X = nullptr;                 // [nchans][xpitch] spectra
     float* xreal = nullptr;              // [nchans][nfft] unpacked series (out-of-place R2C input)
+    bool r2c_inplace = false;            // large plans: the series are unpacked into X's rows instead
     long long xpitch = 0;
     float2* Y = nullptr;                 // TIME mode: [y_rows][ypitch] (lazily allocated)
     long long ypitch = 0;
@@ -298,8 +299,11 @@ int make_fft_plans(fdd_plan* p)
     p->have_r2c = true;
     if (cufftSetAutoAllocation(p->r2c, 0) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
     long long n[1] = {p->nfft};
-    long long inembed[1] = {p->nfft}, onembed[1] = {p->xpitch};
-    if (cufftMakePlanMany64(p->r2c, 1, n, inembed, 1, p->nfft, onembed, 1, p->xpitch,
+    // (in place, for plans whose unpacked copy alone would take 16 GiB - the paper's 2^23-point series:
+    //  real rows of pitch 2 xpitch floats inside X's own rows)
+    const long long rpitch = p->r2c_inplace ? 2 * p->xpitch : p->nfft;
+    long long inembed[1] = {rpitch}, onembed[1] = {p->xpitch};
+    if (cufftMakePlanMany64(p->r2c, 1, n, inembed, 1, rpitch, onembed, 1, p->xpitch,
                             CUFFT_R2C, p->nchans, &ws_r2c) != CUFFT_SUCCESS)
         return FDD_ERR_CUFFT;
     p->fft_ws_bytes = ws_r2c;
@@ -526,8 +530,12 @@ int create_common(fdd_plan* p)
     p->ndm_pad = (int)round_up(p->ndm, fdd::kGenDT);
     int rc = dev_alloc(p, &p->X, (size_t)p->nchans * p->xpitch);
     if (rc != FDD_OK) return rc;
-    rc = dev_alloc(p, &p->xreal, (size_t)p->nchans * p->nfft);
-    if (rc != FDD_OK) return rc;
+    p->r2c_inplace = (size_t)p->nchans * (size_t)p->nfft * sizeof(float) >= ((size_t)16 << 30);
+    if (const char* e = getenv("FDD_R2C_INPLACE")) p->r2c_inplace = atoi(e) != 0;     // (tests)
+    if (!p->r2c_inplace) {
+        rc = dev_alloc(p, &p->xreal, (size_t)p->nchans * p->nfft);
+        if (rc != FDD_OK) return rc;
+    }
     rc = dev_alloc(p, &p->phase64, (size_t)p->nchans * p->ndm_pad);
     if (rc != FDD_OK) return rc;
     p->rec_pshift = 0;
@@ -579,20 +587,23 @@ struct StageTimer {
 };
 
 // time tiles [tile0, tile0 + ntiles) of 64 samples (ntiles < 0: all of them)
+// xdst: the spectra buffer the R2C of this series will write (its rows hold the series first when the
+// plan transforms in place)
 int launch_unpack(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, long long tile0 = 0,
-                  long long ntiles = -1)
+                  long long ntiles = -1, float2* xdst = nullptr)
 {
     if (ntiles < 0) ntiles = (p->nfft + fdd::kUnpackTile - 1) / fdd::kUnpackTile;
     if (ntiles == 0) return FDD_OK;
     dim3 grid((unsigned)ntiles, (unsigned)((p->nchans + fdd::kUnpackTile - 1) / fdd::kUnpackTile));
-    float* xf = p->xreal;
+    float* xf = p->r2c_inplace ? reinterpret_cast<float*>(xdst ? xdst : p->X) : p->xreal;
+    const long long rpitch = p->r2c_inplace ? 2 * p->xpitch : p->nfft;
     const bool vec = (p->nchans % 4 == 0) && ((uintptr_t)in_u8 % 4 == 0);
     if (vec)
         fdd::k_unpack_transpose<4><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        p->nfft, p->offset, tile0);
+                                                        rpitch, p->offset, tile0);
     else
         fdd::k_unpack_transpose<1><<<grid, 256, 0, s>>>(in_u8, xf, p->nchans, p->nsamps, p->nfft,
-                                                        p->nfft, p->offset, tile0);
+                                                        rpitch, p->offset, tile0);
     return cudaGetLastError() == cudaSuccess ? FDD_OK : FDD_ERR_CUDA;
 }
 
@@ -805,7 +816,8 @@ int run_pre(fdd_plan* p, const unsigned char* in_u8, cudaStream_t s, StageTimer&
     if (rc != FDD_OK) return rc;
     tm.begin(FDD_STAGE_R2C, 1);
     if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-    if (cufftExecR2C(p->r2c, p->xreal, p->X) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
+    if (cufftExecR2C(p->r2c, p->r2c_inplace ? reinterpret_cast<float*>(p->X) : p->xreal, p->X) != CUFFT_SUCCESS)
+        return FDD_ERR_CUFFT;
     const int rcp = launch_pad_add_rect(p, p->X, s);
     tm.end();
     return rcp;
@@ -1255,12 +1267,14 @@ int fdd_execute_beams(fdd_plan* p, const unsigned char* in_u8, void* out, int nb
         for (int b = 0; b < gb; ++b) {
             // a2 + a3 of beam b0 + b into its slot of beam_X
             tm.begin(FDD_STAGE_UNPACK, 1);
-            rc = launch_unpack(p, in_u8 + (size_t)(b0 + b) * in_beam, s);
+            rc = launch_unpack(p, in_u8 + (size_t)(b0 + b) * in_beam, s, 0, -1, p->beam_X + (long long)b * xstride);
             tm.end();
             if (rc != FDD_OK) return rc;
             tm.begin(FDD_STAGE_R2C, 1);
             if (cufftSetStream(p->r2c, s) != CUFFT_SUCCESS) return FDD_ERR_CUFFT;
-            if (cufftExecR2C(p->r2c, p->xreal, p->beam_X + (long long)b * xstride) != CUFFT_SUCCESS)
+            if (cufftExecR2C(p->r2c,
+                             p->r2c_inplace ? reinterpret_cast<float*>(p->beam_X + (long long)b * xstride) : p->xreal,
+                             p->beam_X + (long long)b * xstride) != CUFFT_SUCCESS)
                 return FDD_ERR_CUFFT;
             rc = launch_pad_add_rect(p, p->beam_X + (long long)b * xstride, s);
             tm.end();

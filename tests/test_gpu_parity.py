@@ -786,3 +786,24 @@ def test_inverse_transform_choices(F, oracle_c, nchans, nsamps, ndm, step, kerne
             print("inverse", which, kernel, nchans, nsamps, worst)
         with pytest.raises(F.FddError):
             plan.set_inverse(7)
+
+
+def test_in_place_forward_transform(F, oracle_c, monkeypatch):
+    """Plans whose unpacked copy alone would take 16 GiB (the paper's 2^23-point series) unpack into the
+    spectra buffer and transform in place; FDD_R2C_INPLACE forces that layout at a test size, through
+    fdd_execute, fdd_execute_host and fdd_execute_beams."""
+    import torch
+    monkeypatch.setenv("FDD_R2C_INPLACE", "1")
+    w = synth.small_workload(77, 40, 3000, 70, dm_step=0.6)
+    u8 = synth.make_filterbank(w)
+    ref = O.fdd_rows(u8, _delays_for(w), range(w.ndm), mode="time")
+    with _plan_for(F, w) as plan:
+        parity.assert_rows(_run(F, plan, u8, "time"), ref, "time", "in-place R2C")
+        h_out = torch.empty((plan.ndm, plan.nsamps), dtype=torch.float32).pin_memory()
+        plan.execute_host(u8, h_out, F.FDD_MODE_TIME)
+        parity.assert_rows(h_out.numpy(), ref, "time", "in-place R2C, host")
+        beams = np.stack([u8, u8[::-1].copy()])
+        out = torch.empty((2, plan.ndm, plan.nsamps), dtype=torch.float32, device="cuda")
+        plan.execute_beams(torch.from_numpy(beams).cuda(), out, 2, F.FDD_MODE_TIME)
+        torch.cuda.synchronize()
+        parity.assert_rows(out[0].cpu().numpy(), ref, "time", "in-place R2C, beams")
