@@ -62,7 +62,8 @@ enum fdd_status {
     FDD_ERR_ALLOC = -2,
     FDD_ERR_CUDA = -3,
     FDD_ERR_CUFFT = -4,
-    FDD_ERR_UNSUPPORTED = -5
+    FDD_ERR_UNSUPPORTED = -5,
+    FDD_ERR_TOO_LARGE = -6     /* fdd_rotate_sum_static: the problem does not fit the static scratch */
 };
 
 /* Kernel choice for step a4 (fdd_plan_set_kernel). */
@@ -281,6 +282,33 @@ int fdd_measure_fp32_peak(int packed, int iters, double *tflops_host, float *ms_
  * a_f16_dev[128][64] and b_f16_dev[64][64] (IEEE half, row-major, DEVICE), through the shared-memory
  * operand layout, descriptors, tcgen05.mma sequence and TMEM read-out FDD_KERNEL_TENSOR uses. */
 int fdd_tc_selftest(const void *a_f16_dev, const void *b_f16_dev, float *d_dev, void *cuda_stream);
+
+/* Step a4 WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it):
+ *   out[j][k] = sum_c X[c][k] exp(+2 pi i k d[j][c] / nfft)  (+ dc_add on Re out[j][0])
+ * (Eq. 4 + Eq. 7; the sum FDD_MODE_FOURIER returns, any delay table).  No plan:
+ *   x_dev       DEVICE, complex64 [nchans][xpitch], bins 0 .. nbins-1 of every channel's spectrum
+ *               (xpitch >= nbins, in complex elements), e.g. what fdd_plan_get_spectrum returns
+ *   delays_dev  DEVICE, fp64 [ndm][nchans], delays in samples (any sign, fractional)
+ *   nfft        length of the transform the spectra come from (a power of two gives exact phases);
+ *               nbins <= nfft / 2 + 1
+ *   out_dev     DEVICE, complex64 [ndm][nbins], overwritten
+ *   dc_add      added to the real part of bin 0 of every trial DM (the mean step a2 removed, or 0)
+ * Caller owns every buffer; the call is asynchronous on cuda_stream (two kernels) and runs on the
+ * CURRENT device, which must own the buffers.  Its only scratch - the 64-bit phase steps
+ * frac(d / nfft) 2^64, [nchans][ndm rounded up to 8] - is a static __device__ array of
+ * FDD_STATIC_MAX_PHASES entries (8 MiB, held by every GPU that loads the library until the process
+ * exits); the call calls no cudaMalloc / cudaFree / allocating library routine (its first call on a
+ * device looks the array's address up, once).  Limits and errors: FDD_ERR_TOO_LARGE if
+ * nchans * round_up(ndm, 8) > FDD_STATIC_MAX_PHASES (e.g. 1024 channels x 1024 trial DMs fit) or the
+ * grid would exceed 2^31 - 1 CTAs; FDD_ERR_INVALID_ARG for NULL pointers or non-positive sizes;
+ * FDD_ERR_CUDA.  The array is shared by every call on a device and rewritten by each: calls that
+ * overlap on the GPU (different streams or host threads) RACE - serialise them.  Speed: that of
+ * FDD_KERNEL_GENERIC (one fresh phasor per element); plans remain the fast path. */
+#define FDD_STATIC_MAX_PHASES 1048576
+int fdd_rotate_sum_static(const void *x_dev, long long xpitch, const double *delays_dev, int nchans,
+                          long long nbins, long long nfft, int ndm, void *out_dev, float dc_add,
+                          void *cuda_stream);
 
 const char *fdd_error_string(int status);
 

@@ -19,6 +19,8 @@ FDD_KERNEL_MIXED = 4
 FDD_KERNEL_TENSOR = 5
 FDD_INVERSE_CUFFT, FDD_INVERSE_TWO_PASS = 0, 1
 FDD_OK = 0
+FDD_ERR_TOO_LARGE = -6
+FDD_STATIC_MAX_PHASES = 1 << 20
 FDD_NUM_STAGES = 6
 STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift_add")
 
@@ -29,7 +31,7 @@ EXPORTS = (
     "fdd_execute", "fdd_execute_host", "fdd_execute_beams", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_plan_get_padding", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
-    "fdd_error_string",
+    "fdd_rotate_sum_static", "fdd_error_string",
 )
 
 
@@ -78,6 +80,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_rotate_sum_only.argtypes = [vp, vp, c_int, vp]
     lib.fdd_plan_get_padding.argtypes = [vp, P(c_ll)]
     lib.fdd_tc_selftest.argtypes = [vp, vp, vp, vp]
+    lib.fdd_rotate_sum_static.argtypes = [vp, c_ll, vp, c_int, c_ll, c_ll, c_int, vp, ctypes.c_float, vp]
     lib.fdd_measure_fp32_peak.argtypes = [c_int, c_int, P(c_dbl), P(ctypes.c_float)]
     for name in EXPORTS:
         getattr(lib, name).restype = c_int
@@ -280,3 +283,13 @@ def tc_selftest(a_f16, b_f16, d_out, stream=None) -> None:
     """d_out[128][64] f32 = a_f16[128][64] @ b_f16[64][64].T on the tcgen05 path (device tensors)."""
     _check(load_library().fdd_tc_selftest(_ptr(a_f16), _ptr(b_f16), _ptr(d_out), _stream_handle(stream)),
            "fdd_tc_selftest")
+
+
+def rotate_sum_static(x_dev, xpitch: int, delays_dev, nchans: int, nbins: int, nfft: int, ndm: int, out_dev,
+                      dc_add: float = 0.0, stream=None) -> None:
+    """Step a4 without any allocation (scratch in a static device array of FDD_STATIC_MAX_PHASES entries):
+    out_dev[ndm][nbins] c64 = sum over channels of x_dev[nchans][xpitch] c64 rotated by delays_dev[ndm][nchans]
+    f64 (device tensors or addresses).  Calls that overlap on the GPU race: include/fdd.h."""
+    _check(load_library().fdd_rotate_sum_static(_ptr(x_dev), int(xpitch), _ptr(delays_dev), int(nchans), int(nbins),
+                                                int(nfft), int(ndm), _ptr(out_dev), float(dc_add),
+                                                _stream_handle(stream)), "fdd_rotate_sum_static")

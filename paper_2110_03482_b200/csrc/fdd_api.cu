@@ -1446,6 +1446,7 @@ const char* fdd_error_string(int status)
         case FDD_ERR_CUDA: return "CUDA error";
         case FDD_ERR_CUFFT: return "cuFFT error";
         case FDD_ERR_UNSUPPORTED: return "unsupported";
+        case FDD_ERR_TOO_LARGE: return "problem larger than the static scratch (FDD_STATIC_MAX_PHASES)";
         default: return "unknown status";
     }
 }
