@@ -33,7 +33,16 @@ constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per
 constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
 constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
-constexpr int kIfftBatch = 16;                        // rows per pass of the own inverse (ring: 2 x 64 MiB at 2^20)
+// rows per pass of the own inverse (ring: 2 x 64 MiB at 2^20); FDD_IFFT_BATCH for experiments
+int ifft_batch()
+{
+    static const int n = [] {
+        const char* e = getenv("FDD_IFFT_BATCH");
+        const int v = e ? atoi(e) : 0;
+        return v >= 1 && v <= 4096 ? v : 16;
+    }();
+    return n;
+}
 constexpr int kTensorMinRows = 1024;                  // launches with fewer trial DMs take the FP32 kernels
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
@@ -106,7 +115,7 @@ struct fdd_plan {
     int inverse_request = FDD_INVERSE_CUFFT;
     bool ifft_on = false;                // decided with the TIME-mode resources
     bool dc_in_bin0 = true;              // a4 restores the mean in bin 0 (false: the own inverse adds it)
-    float2* ifft_ring = nullptr;         // [2][kIfftBatch][nfft_out / 2]
+    float2* ifft_ring = nullptr;         // [2][ifft_batch()][nfft_out / 2]
     size_t ifft_ring_bytes = 0;
     // multi-beam execution (fdd_execute_beams): spectra and TIME-mode sums of one group of beams
     float2* beam_X = nullptr;            // [beam_group][nchans][xpitch]
@@ -469,7 +478,7 @@ int ensure_time_family(fdd_plan* p, int* family_out)
     int m1, m2;
     p->ifft_on = family == 0 && p->inverse_request == FDD_INVERSE_TWO_PASS && fdd::ifft_split(p->nfft_out, &m1, &m2);
     if (p->ifft_on && !p->ifft_ring) {
-        const size_t n = (size_t)2 * kIfftBatch * (size_t)(p->nfft_out / 2);
+        const size_t n = (size_t)2 * ifft_batch() * (size_t)(p->nfft_out / 2);
         if ((rc = dev_alloc(p, &p->ifft_ring, n)) != FDD_OK) return rc;
         p->ifft_ring_bytes = n * sizeof(float2);
     }
@@ -764,8 +773,8 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
         const float mean = p->padded ? 0.f
                                      : (float)((double)p->offset * (double)p->nchans * (double)p->nsamps / (double)p->nfft);
         const int rc = fdd::ifft_launch(ysrc, p->ypitch, rows, dst, p->nsamps_out, p->nsamps_out, p->nfft_out, mean,
-                                        p->ifft_ring, kIfftBatch, s);
-        *launches += 2 * ((rows + kIfftBatch - 1) / kIfftBatch);
+                                        p->ifft_ring, ifft_batch(), s);
+        *launches += 2 * ((rows + ifft_batch() - 1) / ifft_batch());
         return rc == 0 ? FDD_OK : (rc == -5 ? FDD_ERR_UNSUPPORTED : FDD_ERR_CUDA);
     }
     const bool direct = (p->nsamps_out == p->nfft_out);

@@ -9,248 +9,384 @@
 //   pass A  B[n1][k2] = e^{+2 pi i k2 n1 / M} sum_k1 Z[M2 k1 + k2] e^{+2 pi i k1 n1 / M1}
 //   pass B  z[n1 + M1 n2] = sum_k2 B[n1][k2] e^{+2 pi i k2 n2 / M2}
 //
-// Pass A reads Y once (its own 64-byte run of 8 bins k2 and the mirrored run, for every k1), forms Z on
+// Pass A reads Y once (its own run of C adjacent bins k2 and the mirrored run, for every k1), forms Z on
 // the fly - cuFFT's C2R spends a pass of its own on that - and writes B; pass B reads B, and writes the
 // real series once, adding the mean of the series that step a4 then leaves out of bin 0 (the fp32
 // transform works on a series of rms sigma instead of 256 sigma).  B lives in a small ring that both
-// passes go through batch by batch (16 rows = 64 MiB at 2^20 points), so that it can stay in the 126 MB
-// L2 and HBM sees Y once and y once.
+// passes go through batch by batch, so that it can stay in the 126 MB L2 and HBM sees Y once and y once.
 //
-// Status (FDD_INVERSE_TWO_PASS, not the default): correct for every length and crop the tests cover and
-// about 2x more accurate than the cuFFT path, but 56 ms against cuFFT's 21 ms at 4096 x 2^20 on B200:
-// the radix-4 shared-memory stages are instruction- and latency-bound (an fp32 transform of this size
-// needs ~5 ms of FMA-pipe time at best; cuFFT's two passes sit at 70 % of their HBM roofline).
-//
-// Both passes run the same shared-memory kernel: a tile of L x 8 complex (L = M1 or M2 points of 8
-// independent transforms side by side, row pitch 9 so that transposed accesses spread over the banks),
-// in-place decimation-in-frequency radix-4 stages (+ one radix-2), results read out in digit-reversed
-// order.
+// Both passes run the same transform of L = M1 or M2 points, C of them side by side in a CTA (C adjacent
+// columns = one run of 8 C bytes per global row): a Stockham autosort transform whose radix-8 butterflies
+// live in registers - a thread holds the 8 points t + q L / 8, q < 8, of one column; between stages the
+// points are exchanged through a shared-memory tile [L][C + 1]; log2 L not a multiple of 3: one radix-2
+// or radix-4 stage first (Ns = 1, no twiddles).  The first stage loads straight from global memory and
+// the last one stores straight to it.  Round 2's first version kept the data in shared memory and ran
+// radix-4 stages there: 56 ms at 4096 x 2^20 against cuFFT's 21 ms (instruction- and latency-bound).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 namespace fdd {
-
-constexpr int kIfftC = 8;              // transforms side by side in a tile
-constexpr int kIfftPitch = 9;          // float2 per tile row
-constexpr int kIfftThreads = 256;
-constexpr int kIfftMaxL = 2048;
-
-// tile + stage twiddles + (pass A) half-angle table and the per-column twiddle tables
-__host__ __device__ inline size_t ifft_smem_bytes(int L)
-{
-    return ((size_t)L * (kIfftPitch + 2) + kIfftC * 97) * sizeof(float2);
-}
-
-// position `pos` of the in-place transform holds output index ifft_outidx(pos): the digits of pos
-// (one base-4 digit per radix-4 stage, most significant = first stage, then one bit if log2 L is odd)
-// in reverse order.  lgL = log2 L.
-__device__ __forceinline__ int ifft_outidx(int pos, int lgL)
-{
-    const int nb = lgL & ~1;                                   // bits in the base-4 digits
-    const unsigned x = (unsigned)pos >> (lgL & 1);
-    unsigned r = nb ? __brev(x) >> (32 - nb) : 0u;             // bit reversal ...
-    r = ((r & 0xAAAAAAAAu) >> 1) | ((r & 0x55555555u) << 1);   // ... with the two bits of a digit swapped back
-    return (int)(r | (((unsigned)pos & (unsigned)(lgL & 1)) << nb));
-}
 
 __device__ __forceinline__ float2 ifft_cmul(float2 a, float2 b)
 {
     return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
+__device__ __forceinline__ float2 ifft_add(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 ifft_sub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 
-// tw[j] = e^{+2 pi i j / L}, j < L (in shared memory); s = tile [L][kIfftPitch]
-__device__ __forceinline__ void ifft_tile(float2* s, const float2* tw, int lgL)
+// Butterflies with the kernel e^{+2 pi i p q / R}, in place, outputs in natural order
+__device__ __forceinline__ void ifft_bf2(float2& a, float2& b)
 {
-    const int L = 1 << lgL;
-    int lgspan = lgL;
-    while (lgspan >= 2) {
-        const int span = 1 << lgspan, str = span >> 2;
-        const int lgt = lgL - lgspan;                          // twiddle index step = L / span
-        for (int w = threadIdx.x; w < (L >> 2) * kIfftC; w += kIfftThreads) {
-            const int col = w & (kIfftC - 1), g = w >> 3;
-            const int i = g & (str - 1), blk = g >> (lgspan - 2);
-            float2* p = s + ((blk << lgspan) + i) * kIfftPitch + col;
-            const float2 a0 = p[0], a1 = p[str * kIfftPitch], a2 = p[2 * str * kIfftPitch], a3 = p[3 * str * kIfftPitch];
-            // radix-4, kernel e^{+2 pi i p q / 4}
-            const float2 s02 = make_float2(a0.x + a2.x, a0.y + a2.y), d02 = make_float2(a0.x - a2.x, a0.y - a2.y);
-            const float2 s13 = make_float2(a1.x + a3.x, a1.y + a3.y), d13 = make_float2(a1.x - a3.x, a1.y - a3.y);
-            const float2 b0 = make_float2(s02.x + s13.x, s02.y + s13.y);
-            const float2 b2 = make_float2(s02.x - s13.x, s02.y - s13.y);
-            const float2 b1 = make_float2(d02.x - d13.y, d02.y + d13.x);      // d02 + i d13
-            const float2 b3 = make_float2(d02.x + d13.y, d02.y - d13.x);      // d02 - i d13
-            p[0] = b0;
-            p[str * kIfftPitch] = ifft_cmul(b1, tw[i << lgt]);
-            p[2 * str * kIfftPitch] = ifft_cmul(b2, tw[(2 * i) << lgt]);
-            p[3 * str * kIfftPitch] = ifft_cmul(b3, tw[(3 * i) << lgt]);
+    const float2 t = a;
+    a = ifft_add(t, b);
+    b = ifft_sub(t, b);
+}
+__device__ __forceinline__ void ifft_bf4(float2& y0, float2& y1, float2& y2, float2& y3)
+{
+    const float2 s02 = ifft_add(y0, y2), d02 = ifft_sub(y0, y2);
+    const float2 s13 = ifft_add(y1, y3), d13 = ifft_sub(y1, y3);
+    y0 = ifft_add(s02, s13);
+    y2 = ifft_sub(s02, s13);
+    y1 = make_float2(d02.x - d13.y, d02.y + d13.x);      // d02 + i d13
+    y3 = make_float2(d02.x + d13.y, d02.y - d13.x);      // d02 - i d13
+}
+__device__ __forceinline__ void ifft_bf8(float2 (&v)[8])
+{
+    // X[p] = A[p & 3] + w^p B[p & 3], A = DFT4(even), B = DFT4(odd), w = e^{i pi / 4}
+    ifft_bf4(v[0], v[2], v[4], v[6]);                    // A0..A3 in v[0], v[2], v[4], v[6]
+    ifft_bf4(v[1], v[3], v[5], v[7]);                    // B0..B3 in v[1], v[3], v[5], v[7]
+    const float h = 0.70710678118654752f;
+    const float2 b0 = v[1];
+    const float2 b1 = make_float2((v[3].x - v[3].y) * h, (v[3].x + v[3].y) * h);     // (1 + i) / sqrt 2
+    const float2 b2 = make_float2(-v[5].y, v[5].x);                                  // i
+    const float2 b3 = make_float2(-(v[7].x + v[7].y) * h, (v[7].x - v[7].y) * h);    // (-1 + i) / sqrt 2
+    const float2 a0 = v[0], a1 = v[2], a2 = v[4], a3 = v[6];
+    v[0] = ifft_add(a0, b0); v[4] = ifft_sub(a0, b0);
+    v[1] = ifft_add(a1, b1); v[5] = ifft_sub(a1, b1);
+    v[2] = ifft_add(a2, b2); v[6] = ifft_sub(a2, b2);
+    v[3] = ifft_add(a3, b3); v[7] = ifft_sub(a3, b3);
+}
+
+// The transform of one column: v[q] = point t + q L / 8 of the input on entry; the results are handed
+// to emit(r, index, value), r = 0 .. 7 in turn.  s: tile [rows][C + 1] shared by the CTA's C columns;
+// tw[j] = e^{+2 pi i j / L}.
+// Stockham: a radix-R stage with Ns = product of the earlier radices takes butterfly j (< L / R) from the
+// points j + r L / R, twiddles them by e^{2 pi i r k / (Ns R)}, k = j mod Ns, and puts the outputs at
+// (j - k) R + k + r Ns.  Every CTA thread must call it (it synchronises the CTA).
+// (t_in, c_in): the thread's role up to the first exchange, (t, c) after it - the exchange goes through
+// the tile, so a thread may pick up another part of the work there (pass B loads rows along t and
+// stores along c).  PAD: tile row i sits at i + i / 8, which keeps the first stage's stores of a warp
+// that runs along t off each other's banks.
+template <bool PAD>
+__device__ __forceinline__ int ifft_row(int i) { return PAD ? i + (i >> 3) : i; }
+
+template <int LG, int LGC, bool PAD, class Emit>
+__device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float2* tw, int t_in, int c_in, int t,
+                                          int c, Emit emit)
+{
+    constexpr int L = 1 << LG, T = L / 8, P = (1 << LGC) + 1;
+    constexpr int R0 = 1 << (LG % 3), N8 = LG / 3;
+    bool wrote = false;
+    if (R0 == 2) {
+        // four radix-2 butterflies u: points v[u], v[u + 4] of butterfly j = t + u T -> 2 j, 2 j + 1
+#pragma unroll
+        for (int u = 0; u < 4; ++u) ifft_bf2(v[u], v[u + 4]);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            s[ifft_row<PAD>(2 * (t_in + u * T)) * P + c_in] = v[u];
+            s[ifft_row<PAD>(2 * (t_in + u * T) + 1) * P + c_in] = v[u + 4];
         }
-        __syncthreads();
-        lgspan -= 2;
+        wrote = true;
+    } else if (R0 == 4) {
+        // two radix-4 butterflies u: points v[u + 2 r] of butterfly j = t + u T -> 4 j + r
+#pragma unroll
+        for (int u = 0; u < 2; ++u) ifft_bf4(v[u], v[u + 2], v[u + 4], v[u + 6]);
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) s[ifft_row<PAD>(4 * (t_in + u * T) + r) * P + c_in] = v[u + 2 * r];
+        wrote = true;
     }
-    if (lgspan == 1) {
-        for (int w = threadIdx.x; w < (L >> 1) * kIfftC; w += kIfftThreads) {
-            const int col = w & (kIfftC - 1), g = w >> 3;
-            float2* p = s + (2 * g) * kIfftPitch + col;
-            const float2 a0 = p[0], a1 = p[kIfftPitch];
-            p[0] = make_float2(a0.x + a1.x, a0.y + a1.y);
-            p[kIfftPitch] = make_float2(a0.x - a1.x, a0.y - a1.y);
-        }
+    if (wrote) {
         __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 8; ++q) v[q] = s[ifft_row<PAD>(t + q * T) * P + c];
+    }
+#pragma unroll
+    for (int i = 0; i < N8; ++i) {
+        const int Ns = R0 << (3 * i);
+        const int tt = wrote ? t : t_in, cc = wrote ? c : c_in;
+        const int k = tt & (Ns - 1);
+        if (Ns > 1) {
+            // w^r, r = 1 .. 7, w = e^{2 pi i k / (8 Ns)}: three from the table, four products
+            const int step = L / (8 * Ns);
+            const float2 w1 = tw[k * step], w2 = tw[2 * k * step], w4 = tw[4 * k * step];
+            const float2 w3 = ifft_cmul(w1, w2), w5 = ifft_cmul(w1, w4), w6 = ifft_cmul(w2, w4);
+            const float2 w7 = ifft_cmul(w3, w4);
+            v[1] = ifft_cmul(v[1], w1); v[2] = ifft_cmul(v[2], w2); v[3] = ifft_cmul(v[3], w3);
+            v[4] = ifft_cmul(v[4], w4); v[5] = ifft_cmul(v[5], w5); v[6] = ifft_cmul(v[6], w6);
+            v[7] = ifft_cmul(v[7], w7);
+        }
+        ifft_bf8(v);
+        const int j0 = (tt - k) * 8 + k;
+        if (i == N8 - 1) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) emit(r, j0 + r * Ns, v[r]);
+        } else {
+            if (wrote) __syncthreads();              // the reads of the stage before are done
+#pragma unroll
+            for (int r = 0; r < 8; ++r) s[ifft_row<PAD>(j0 + r * Ns) * P + cc] = v[r];
+            wrote = true;
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = s[ifft_row<PAD>(t + q * T) * P + c];
+        }
     }
 }
 
-__device__ __forceinline__ void ifft_make_twiddles(float2* tw, int L)
+// tw[j] = e^{+2 pi i j / L}, j < L (the quotient is exact in fp32)
+__device__ __forceinline__ void ifft_make_twiddles(float2* tw, int L, int nthreads)
 {
-    for (int j = threadIdx.x; j < L; j += kIfftThreads) {
+    for (int j = threadIdx.x; j < L; j += nthreads) {
         float sn, cs;
         sincospif(2.f * (float)j / (float)L, &sn, &cs);
         tw[j] = make_float2(cs, sn);
     }
 }
 
-// Pass A.  grid = (M2 / 8, rows).  Y: [rows][ypitch] sums of a4 (bins 0 .. M); B: [rows][M] as [n1][k2].
-// Twiddles come from small per-CTA tables (a sincospif per element would cost more than the transform):
-//   e^{i pi k / M},        k = M2 k1 + k2:  half[k1] = e^{i pi k1 / M1}  times  e^{i pi k2 / M}
-//   e^{2 pi i k2 n1 / M},  n1 = 32 a + b:   hi[c][a] = e^{2 pi i k2 32 a / M}  times  lo[c][b] = e^{2 pi i k2 b / M}
-__global__ void __launch_bounds__(kIfftThreads)
-k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg1, int lg2)
+__host__ __device__ constexpr int ifft_hi_len(int lg) { return lg > 5 ? 1 << (lg - 5) : 1; }
+
+// shared memory of the two passes, in float2 elements
+constexpr size_t ifft_smem_a(int lg, int lgc)
 {
+    return ((size_t)(1 << lg) * ((1 << lgc) + 1) + 2 * (size_t)(1 << lg) + (size_t)(1 << lgc) * (ifft_hi_len(lg) + 34)) *
+           sizeof(float2);
+}
+constexpr size_t ifft_smem_b(int lg, int lgc)
+{
+    return ((size_t)((1 << lg) + (1 << lg) / 8) * ((1 << lgc) + 1) + (size_t)(1 << lg)) * sizeof(float2);   // padded rows
+}
+
+// Pass A.  grid = (M2 / C, rows), CTA = C columns x L / 8 threads, L = M1 = 2^LG.
+// Y: [rows][ypitch] sums of a4 (bins 0 .. M); B: [rows][M] as [n1][k2].
+// Twiddles come from small per-CTA tables (a sincospif per element would cost as much as the transform):
+//   e^{i pi k / M},        k = M2 k1 + k2:  half[k1] = e^{i pi k1 / M1}  times  colw[c] = e^{i pi k2 / M}
+//   e^{2 pi i k2 n1 / M},  n1 = 32 a + b:   hi[c][a] = e^{2 pi i k2 32 a / M}  times  lo[c][b] = e^{2 pi i k2 b / M}
+template <int LG, int LGC>
+__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : 2)
+k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg2)
+{
+    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, P = C + 1, NT = T * C, HI = ifft_hi_len(LG);
     extern __shared__ float2 ifft_smem[];
-    const int M1 = 1 << lg1, M2 = 1 << lg2;
-    float2* s = ifft_smem;
-    float2* tw = s + (size_t)M1 * kIfftPitch;
-    float2* half = tw + M1;                        // [M1]
-    float2* hi = half + M1;                        // [8][64]
-    float2* lo = hi + kIfftC * 64;                 // [8][32]
-    float2* colw = lo + kIfftC * 32;               // [8] e^{i pi k2 / M}
-    const long long M = (long long)1 << (lg1 + lg2);
+    float2* s = ifft_smem;                         // [L][P]
+    float2* tw = s + L * P;                        // [L]
+    float2* half = tw + L;                         // [L]
+    float2* hi = half + L;                         // [C][HI]
+    float2* lo = hi + C * HI;                      // [C][32]
+    float2* colw = lo + C * 32;                    // [C] e^{i pi k2 / M}
+    float2* colg = colw + C;                       // [C] e^{2 pi i k2 (L / 8) / M}
+    const int c = threadIdx.x & (C - 1), t = threadIdx.x >> LGC;
+    const long long M = (long long)1 << (LG + lg2);
     const float2* y = Y + (long long)blockIdx.y * ypitch;
     float2* b = B + (long long)blockIdx.y * M;
-    const int c0 = blockIdx.x * kIfftC;
-    ifft_make_twiddles(tw, M1);
+    const int c0 = blockIdx.x * C;
+    // the loads first: they are in flight while the tables are made
+    float2 v[8], m[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const long long k = ((long long)(t + q * T) << lg2) + c0 + c;
+        v[q] = y[k];
+        m[q] = y[M - k];
+    }
+    ifft_make_twiddles(tw, L, NT);
     const float inv_m = 1.f / (float)M;
-    for (int j = threadIdx.x; j < M1; j += kIfftThreads) {
+    for (int j = threadIdx.x; j < L; j += NT) {
         float sn, cs;
-        sincospif((float)j / (float)M1, &sn, &cs);
+        sincospif((float)j / (float)L, &sn, &cs);
         half[j] = make_float2(cs, sn);
     }
-    for (int j = threadIdx.x; j < kIfftC * 96; j += kIfftThreads) {
-        const int c = j / 96, r = j - c * 96;
-        const long long k2 = c0 + c;
+    for (int j = threadIdx.x; j < C * (HI + 32); j += NT) {
+        const int cc = j / (HI + 32), r = j - cc * (HI + 32);
+        const long long k2 = c0 + cc;
         float sn, cs;
-        if (r < 64) {                              // exact arguments: k2 * 32 a < M2 * M1 = M <= 2^22
+        if (r < HI) {                              // exact arguments: k2 * 32 a < M2 * M1 = M <= 2^22
             sincospif(2.f * (float)(k2 * 32 * r) * inv_m, &sn, &cs);
-            hi[c * 64 + r] = make_float2(cs, sn);
+            hi[cc * HI + r] = make_float2(cs, sn);
         } else {
-            sincospif(2.f * (float)(k2 * (r - 64)) * inv_m, &sn, &cs);
-            lo[c * 32 + (r - 64)] = make_float2(cs, sn);
+            sincospif(2.f * (float)(k2 * (r - HI)) * inv_m, &sn, &cs);
+            lo[cc * 32 + (r - HI)] = make_float2(cs, sn);
         }
     }
-    if (threadIdx.x < kIfftC) {
+    if (threadIdx.x < C) {
         float sn, cs;
         sincospif((float)(c0 + threadIdx.x) * inv_m, &sn, &cs);
         colw[threadIdx.x] = make_float2(cs, sn);
+        sincospif(2.f * (float)((long long)(c0 + threadIdx.x) * T) * inv_m, &sn, &cs);
+        colg[threadIdx.x] = make_float2(cs, sn);
     }
     __syncthreads();
-    for (int e = threadIdx.x; e < M1 * kIfftC; e += kIfftThreads) {
-        const int k1 = e >> 3, c = e & (kIfftC - 1);
-        const long long k = ((long long)k1 << lg2) + c0 + c;
-        const float2 a = y[k];
-        float2 m = y[M - k];
-        m.y = -m.y;                                // conj Y[M - k]
-        const float2 w = ifft_cmul(half[k1], colw[c]);      // e^{+2 pi i k / N}
-        const float2 sum = make_float2(a.x + m.x, a.y + m.y), dif = make_float2(a.x - m.x, a.y - m.y);
-        const float2 wd = ifft_cmul(w, dif);
-        s[k1 * kIfftPitch + c] = make_float2(sum.x - wd.y, sum.y + wd.x);         // sum + i w dif
+    // e^{+2 pi i k / N} = e^{i pi k1 / M1} e^{i pi k2 / M}, k1 = t + q L / 8: half[t] colw[c] times e^{i pi q / 8}
+    const float2 w0 = ifft_cmul(half[t], colw[c]);
+    const float kc[8] = {1.f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f,
+                         0.f, -0.38268343236508977f, -0.70710678118654752f, -0.92387953251128674f};
+    const float ks[8] = {0.f, 0.38268343236508977f, 0.70710678118654752f, 0.92387953251128674f,
+                         1.f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f};
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const float2 a = v[q];
+        const float2 mc = make_float2(m[q].x, -m[q].y);                  // conj Y[M - k]
+        const float2 w = ifft_cmul(w0, make_float2(kc[q], ks[q]));
+        const float2 wd = ifft_cmul(w, ifft_sub(a, mc));
+        const float2 sum = ifft_add(a, mc);
+        v[q] = make_float2(sum.x - wd.y, sum.y + wd.x);                  // sum + i w dif
     }
-    __syncthreads();
-    ifft_tile(s, tw, lg1);
-    for (int e = threadIdx.x; e < M1 * kIfftC; e += kIfftThreads) {
-        const int pos = e >> 3, c = e & (kIfftC - 1);
-        const int n1 = ifft_outidx(pos, lg1);
-        const float2 w = ifft_cmul(hi[c * 64 + (n1 >> 5)], lo[c * 32 + (n1 & 31)]);   // e^{+2 pi i k2 n1 / M}
-        b[((long long)n1 << lg2) + c0 + c] = ifft_cmul(s[pos * kIfftPitch + c], w);
-    }
+    // e^{+2 pi i k2 n1 / M} for the outputs n1 = t + r L / 8 in turn: the first from the hi / lo tables, then
+    // times colg[c] each
+    float2 pw = ifft_cmul(hi[c * HI + (t >> 5)], lo[c * 32 + (t & 31)]);
+    const float2 pg = colg[c];
+    float2* bc = b + c0 + c;
+    ifft_core<LG, LGC, false>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
+        if (r > 0) pw = ifft_cmul(pw, pg);
+        bc[(long long)n1 << lg2] = ifft_cmul(val, pw);
+    });
 }
 
-// Pass B.  grid = (M1 / 8, rows).  out: [rows][opitch] floats, the first nout of the 2 M samples.
-__global__ void __launch_bounds__(kIfftThreads)
+// Pass B.  grid = (M1 / C, rows), CTA = C rows n1 of B x L / 8 threads, L = M2 = 2^LG.
+// out: [rows][opitch] floats, the first nout of the 2 M samples.
+template <int LG, int LGC>
+__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : 2)
 k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long opitch, long long nout, int lg1,
-              int lg2, float mean)
+              float mean)
 {
+    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, P = C + 1, NT = T * C;
     extern __shared__ float2 ifft_smem[];
-    const int M2 = 1 << lg2;
-    float2* s = ifft_smem;
-    float2* tw = ifft_smem + (size_t)M2 * kIfftPitch;
-    const long long M = (long long)1 << (lg1 + lg2);
-    const float2* b = B + (long long)blockIdx.y * M;
+    float2* s = ifft_smem;                         // [L + L / 8][P] (padded rows)
+    float2* tw = s + (L + L / 8) * P;              // [L]
+    // loads (and the first stage) with the warps along a row of B, the rest and the stores with them across
+    // the C rows: both sides of the transposition this pass is are then runs of whole sectors
+    const int c = threadIdx.x & (C - 1), t = threadIdx.x >> LGC;
+    const int t_in = LG > 3 ? (int)(threadIdx.x & (T - 1)) : t, c_in = LG > 3 ? (int)(threadIdx.x >> (LG - 3)) : c;
+    const long long M = (long long)1 << (LG + lg1);
+    const long long n1 = (long long)blockIdx.x * C + c;
+    const float2* b = B + (long long)blockIdx.y * M + (((long long)blockIdx.x * C + c_in) << LG);
     float* o = out + (long long)blockIdx.y * opitch;
-    const int n10 = blockIdx.x * kIfftC;
-    ifft_make_twiddles(tw, M2);
-    for (int e = threadIdx.x; e < M2 * kIfftC; e += kIfftThreads) {
-        const int r = e >> lg2, k2 = e & (M2 - 1);                                // consecutive lanes: consecutive k2
-        s[k2 * kIfftPitch + r] = b[((long long)(n10 + r) << lg2) + k2];
-    }
+    float2 v[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = b[t_in + q * T];
+    ifft_make_twiddles(tw, L, NT);
     __syncthreads();
-    ifft_tile(s, tw, lg2);
-    for (int e = threadIdx.x; e < M2 * kIfftC; e += kIfftThreads) {
-        const int pos = e >> 3, r = e & (kIfftC - 1);
-        const long long n = (long long)n10 + r + ((long long)ifft_outidx(pos, lg2) << lg1);   // z[n] = (y[2n], y[2n+1])
-        const float2 v = s[pos * kIfftPitch + r];
+    // (rows of the caller's array may start on an odd float: then two 4-byte stores per point)
+    const bool vec = (reinterpret_cast<uintptr_t>(o) & 7) == 0;
+    ifft_core<LG, LGC, true>(v, s, tw, t_in, c_in, t, c, [&](int, int n2, float2 val) {
+        const long long n = n1 + ((long long)n2 << lg1);                 // z[n] = (y[2n], y[2n+1])
         if (2 * n + 1 < nout) {
-            // (rows of the caller's array may start on an odd float: two 4-byte stores)
-            o[2 * n] = v.x + mean;
-            o[2 * n + 1] = v.y + mean;
+            if (vec) {
+                *reinterpret_cast<float2*>(o + 2 * n) = make_float2(val.x + mean, val.y + mean);
+            } else {
+                o[2 * n] = val.x + mean;
+                o[2 * n + 1] = val.y + mean;
+            }
         } else if (2 * n < nout) {
-            o[2 * n] = v.x + mean;
+            o[2 * n] = val.x + mean;
         }
-    }
+    });
 }
 
-// M = nfft_out / 2 = M1 M2, both powers of two in [8, kIfftMaxL]
+// M = nfft_out / 2 = M1 M2, both powers of two in [8, 2048]
 inline bool ifft_split(long long nfft_out, int* M1, int* M2)
 {
     const long long M = nfft_out / 2;
     if (nfft_out < 128 || (M & (M - 1)) != 0) return false;
     int lg = 0;
     while ((1LL << lg) < M) ++lg;
-    const int l1 = (lg + 1) / 2, l2 = lg - l1;
-    if (l1 > 11 || l2 < 3) return false;
+    // (pass A, whose global rows are runs of C elements, takes the shorter factor: 8 columns in 512 threads
+    //  up to 512 points; pass B reads whole rows)
+    const int l1 = lg / 2, l2 = lg - l1;
+    if (l2 > 11 || l1 < 3) return false;
     *M1 = 1 << l1;
     *M2 = 1 << l2;
     return true;
 }
 
-inline int ifft_set_attributes()
+// columns side by side in a CTA: 8 (64-byte runs of every global row) up to 512 points, 4 above (CTAs of
+// 512 and 1024 threads); FDD_IFFT_WIDE: 8 columns x 1024 points in 1024 threads
+inline int ifft_lgc(int lg)
 {
-    static bool done = false;
-    if (done) return 0;
-    const int bytes = (int)ifft_smem_bytes(kIfftMaxL);
-    if (cudaFuncSetAttribute(k_ifft_pass_a, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(k_ifft_pass_b, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess)
-        return -3;
-    done = true;
+    static const bool wide = getenv("FDD_IFFT_WIDE") != nullptr;
+    return lg <= 9 ? 3 : (lg == 10 && wide ? 3 : 2);
+}
+
+template <int LG, int LGC>
+inline int ifft_launch_a(const float2* Y, long long ypitch, float2* B, int lg2, int rows, cudaStream_t s)
+{
+    static bool attr = false;
+    constexpr size_t bytes = ifft_smem_a(LG, LGC);
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_ifft_pass_a<LG, LGC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
+            cudaSuccess)
+            return -3;
+        attr = true;
+    }
+    k_ifft_pass_a<LG, LGC><<<dim3((unsigned)((1 << lg2) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
+        Y, ypitch, B, lg2);
     return 0;
 }
+
+template <int LG, int LGC>
+inline int ifft_launch_b(const float2* B, float* out, long long opitch, long long nout, int lg1, float mean,
+                         int rows, cudaStream_t s)
+{
+    static bool attr = false;
+    constexpr size_t bytes = ifft_smem_b(LG, LGC);
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_ifft_pass_b<LG, LGC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
+            cudaSuccess)
+            return -3;
+        attr = true;
+    }
+    k_ifft_pass_b<LG, LGC><<<dim3((unsigned)((1 << lg1) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
+        B, out, opitch, nout, lg1, mean);
+    return 0;
+}
+
+#define FDD_IFFT_DISPATCH(lg, lgc, CALL)                       \
+    switch ((lg) * 4 + (lgc)) {                                \
+        case 3 * 4 + 3: { constexpr int LG_ = 3, LGC_ = 3; CALL; break; }   \
+        case 4 * 4 + 3: { constexpr int LG_ = 4, LGC_ = 3; CALL; break; }   \
+        case 5 * 4 + 3: { constexpr int LG_ = 5, LGC_ = 3; CALL; break; }   \
+        case 6 * 4 + 3: { constexpr int LG_ = 6, LGC_ = 3; CALL; break; }   \
+        case 7 * 4 + 3: { constexpr int LG_ = 7, LGC_ = 3; CALL; break; }   \
+        case 8 * 4 + 3: { constexpr int LG_ = 8, LGC_ = 3; CALL; break; }   \
+        case 9 * 4 + 3: { constexpr int LG_ = 9, LGC_ = 3; CALL; break; }   \
+        case 10 * 4 + 2: { constexpr int LG_ = 10, LGC_ = 2; CALL; break; } \
+        case 10 * 4 + 3: { constexpr int LG_ = 10, LGC_ = 3; CALL; break; } \
+        case 11 * 4 + 2: { constexpr int LG_ = 11, LGC_ = 2; CALL; break; } \
+        default: rc = -5;                                      \
+    }
 
 // rows of Y -> rows of out, in batches of `batch` rows through the ring `ring` ([2][batch][M] float2)
 inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
                        long long nfft_out, float mean, float2* ring, int batch, cudaStream_t s)
 {
     int M1, M2;
-    if (!ifft_split(nfft_out, &M1, &M2) || ifft_set_attributes() != 0) return -5;
+    if (!ifft_split(nfft_out, &M1, &M2)) return -5;
     const long long M = (long long)M1 * M2;
     int lg1 = 0, lg2 = 0;
     while ((1 << lg1) < M1) ++lg1;
     while ((1 << lg2) < M2) ++lg2;
+    const int lgc1 = ifft_lgc(lg1), lgc2 = ifft_lgc(lg2);
     int slot = 0;
     for (int r0 = 0; r0 < rows; r0 += batch, slot ^= 1) {
         const int n = rows - r0 < batch ? rows - r0 : batch;
         float2* b = ring + (size_t)slot * batch * M;
-        k_ifft_pass_a<<<dim3((unsigned)(M2 / kIfftC), (unsigned)n), kIfftThreads, ifft_smem_bytes(M1), s>>>(
-            Y + (long long)r0 * ypitch, ypitch, b, lg1, lg2);
-        k_ifft_pass_b<<<dim3((unsigned)(M1 / kIfftC), (unsigned)n), kIfftThreads, ifft_smem_bytes(M2), s>>>(
-            b, out + (long long)r0 * opitch, opitch, nout, lg1, lg2, mean);
+        int rc = 0;
+        FDD_IFFT_DISPATCH(lg1, lgc1, (rc = ifft_launch_a<LG_, LGC_>(Y + (long long)r0 * ypitch, ypitch, b, lg2, n, s)));
+        if (rc != 0) return rc;
+        FDD_IFFT_DISPATCH(lg2, lgc2, (rc = ifft_launch_b<LG_, LGC_>(b, out + (long long)r0 * opitch, opitch, nout,
+                                                                     lg1, mean, n, s)));
+        if (rc != 0) return rc;
     }
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
