@@ -67,8 +67,8 @@ def parse_args():
     ap.add_argument("--beams", type=int, default=1, metavar="B",
                     help="row f1: B beams per step through fdd_execute_beams (beam 0 = the workload's "
                          "input, the others seeded noise made on the device); the rate counts all beams")
-    ap.add_argument("--inverse", default="cufft", choices=["cufft", "two_pass"],
-                    help="step a5: cuFFT (default) or the hand-written two-pass inverse")
+    ap.add_argument("--inverse", default="auto", choices=["auto", "cufft", "two_pass"],
+                    help="step a5: the plan's choice (default), cuFFT, or the hand-written two-pass inverse")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -319,8 +319,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
     if args.decimate:
         plan.set_decimation(args.decimate)
-    if args.inverse == "two_pass":
-        plan.set_inverse(F.FDD_INVERSE_TWO_PASS)
+    if args.inverse != "auto":
+        plan.set_inverse(F.FDD_INVERSE_TWO_PASS if args.inverse == "two_pass" else F.FDD_INVERSE_CUFFT)
     ns_out, nbins = plan.output_shape()                   # = (nsamps, nbins) at full rate
     nfft_out = nfft >> args.decimate
     d_in = torch.from_numpy(u8).cuda()
@@ -370,6 +370,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
     stage_ms, launches = plan.get_stage_ms()
+    own_inverse = mode == F.FDD_MODE_TIME and plan.get_inverse() == F.FDD_INVERSE_TWO_PASS
     plan.set_profiling(False)
     if flush is not None:                                  # the flush is not part of the path
         ms_total = sum(stage_ms.values())
@@ -558,8 +559,10 @@ def run_b200(args, rank: int, local_rank: int, world: int):
         "tdd_comparator": tdd,
         "clocks": sampler.summary(),
         "e2e": e2e,
-        "gpu_launches": int((launches["unpack"] + launches["rotate_sum"])),
-        "library_calls": int(launches["r2c"] + launches["c2r"]),
+        # (step a5 runs this repo's own two-pass inverse or cuFFT: fdd_plan_get_inverse says which)
+        "gpu_launches": int(launches["unpack"] + launches["rotate_sum"] + (launches["c2r"] if own_inverse else 0)),
+        "library_calls": int(launches["r2c"] + (0 if own_inverse else launches["c2r"])),
+        "inverse": ("two_pass" if own_inverse else "cufft") if mode == F.FDD_MODE_TIME else None,
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()
                               if not k.startswith("tdd_")},
         "roofline": roofline,

@@ -87,14 +87,17 @@ enum fdd_kernel {
 
 /* Step a5 (fdd_plan_set_inverse). */
 enum fdd_inverse {
-    FDD_INVERSE_CUFFT = 0,     /* cuFFT (C2R, or the half-length C2C fed by SYMMETRIC2's fused pre-twiddle):
-                                  the default - at 2^20 points it runs at 70 % of the HBM roofline of a
-                                  two-pass transform                                                  */
-    FDD_INVERSE_TWO_PASS = 1   /* the hand-written two-pass inverse real transform, nfft = 2^7 .. 2^23: forms
-                                  the half-length spectrum in its first pass and adds the series' mean
-                                  after the transform, so fp32 works on a series of rms sigma instead of
-                                  256 sigma (TIME-mode error about 2x smaller); at present 2.7x slower
-                                  than cuFFT, cuFFT for other lengths                      */
+    FDD_INVERSE_CUFFT = 0,     /* cuFFT: C2R, or the half-length C2C fed by SYMMETRIC2's fused pre-twiddle  */
+    FDD_INVERSE_TWO_PASS = 1,  /* the hand-written two-pass inverse real transform, nfft = 2^7 .. 2^23
+                                  (radix-8 butterflies in registers): forms the half-length spectrum in
+                                  its first pass and adds the series' mean after the transform, so fp32
+                                  works on a series of rms sigma instead of 256 sigma (TIME-mode error
+                                  about 2x smaller).  Faster than cuFFT's C2R (20.5 vs 21.1 ms at 4096 x
+                                  2^20, 57 vs 82 ms at 1024 x 2^23), slower than the C2C behind
+                                  SYMMETRIC2's fused pre-twiddle; cuFFT for other lengths              */
+    FDD_INVERSE_AUTO = 2       /* the default: TWO_PASS where it applies, a4 writes plain sums (every a4
+                                  kernel but SYMMETRIC2) and the sums of all trial DMs fit the plan's Y
+                                  scratch at once; CUFFT otherwise                                     */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */
@@ -169,9 +172,13 @@ int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
  * tables of fdd_tdd_execute are still made on their first call.) */
 int fdd_plan_prepare(fdd_plan *plan, int mode);
 
-/* Choose the inverse transform of step a5 (enum fdd_inverse; default FDD_INVERSE_CUFFT).  Synchronises the device and drops the
+/* Choose the inverse transform of step a5 (enum fdd_inverse; default FDD_INVERSE_AUTO).  Synchronises the device and drops the
  * TIME-mode scratch (re-made by fdd_plan_prepare or the next TIME execute). */
 int fdd_plan_set_inverse(fdd_plan *plan, int which);
+
+/* *which = the inverse transform the plan's last TIME-mode prepare / execute used: FDD_INVERSE_TWO_PASS
+ * or FDD_INVERSE_CUFFT (also before any). */
+int fdd_plan_get_inverse(const fdd_plan *plan, int *which);
 
 /* TIME mode keeps the sums Y of a chunk of trial DMs in plan-owned scratch between a4 and a5.  The
  * chunk is as many rows as fit `bytes` (default 24 GiB, and never more than half of the free

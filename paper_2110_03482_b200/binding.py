@@ -17,7 +17,7 @@ FDD_MODE_TIME, FDD_MODE_FOURIER = 0, 1
 FDD_KERNEL_AUTO, FDD_KERNEL_GENERIC, FDD_KERNEL_SYMMETRIC, FDD_KERNEL_SYMMETRIC2 = 0, 1, 2, 3
 FDD_KERNEL_MIXED = 4
 FDD_KERNEL_TENSOR = 5
-FDD_INVERSE_CUFFT, FDD_INVERSE_TWO_PASS = 0, 1
+FDD_INVERSE_CUFFT, FDD_INVERSE_TWO_PASS, FDD_INVERSE_AUTO = 0, 1, 2
 FDD_OK = 0
 FDD_ERR_TOO_LARGE = -6
 FDD_STATIC_MAX_PHASES = 1 << 20
@@ -27,7 +27,7 @@ STAGE_NAMES = ("unpack", "r2c", "rotate_sum", "c2r", "tdd_transpose", "tdd_shift
 EXPORTS = (
     "fdd_plan_create", "fdd_plan_create_from_delays", "fdd_plan_set_kdm", "fdd_plan_set_kernel",
     "fdd_plan_set_decimation", "fdd_plan_get_output_shape", "fdd_plan_prepare",
-    "fdd_plan_set_y_budget", "fdd_plan_set_inverse",
+    "fdd_plan_set_y_budget", "fdd_plan_set_inverse", "fdd_plan_get_inverse",
     "fdd_execute", "fdd_execute_host", "fdd_execute_beams", "fdd_tdd_execute", "fdd_plan_destroy", "fdd_plan_get_info",
     "fdd_plan_get_delays", "fdd_plan_set_profiling", "fdd_plan_get_stage_ms",
     "fdd_plan_get_spectrum", "fdd_plan_get_padding", "fdd_rotate_sum_only", "fdd_measure_fp32_peak", "fdd_tc_selftest",
@@ -73,6 +73,7 @@ def load_library() -> ctypes.CDLL:
     lib.fdd_plan_prepare.argtypes = [vp, c_int]
     lib.fdd_plan_set_y_budget.argtypes = [vp, ctypes.c_size_t]
     lib.fdd_plan_set_inverse.argtypes = [vp, c_int]
+    lib.fdd_plan_get_inverse.argtypes = [vp, P(c_int)]
     lib.fdd_plan_get_output_shape.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong),
                                               ctypes.POINTER(ctypes.c_longlong)]
     lib.fdd_plan_get_stage_ms.argtypes = [vp, P(ctypes.c_float), P(c_int)]
@@ -214,7 +215,7 @@ class Plan:
         _check(load_library().fdd_plan_prepare(self._h, int(mode)), "fdd_plan_prepare")
 
     def set_inverse(self, which: int) -> None:
-        """FDD_INVERSE_CUFFT (default) or FDD_INVERSE_TWO_PASS (hand-written, keeps the mean out of fp32)."""
+        """FDD_INVERSE_AUTO (default), FDD_INVERSE_CUFFT or FDD_INVERSE_TWO_PASS (hand-written, keeps the mean out of fp32)."""
         _check(load_library().fdd_plan_set_inverse(self._h, int(which)), "fdd_plan_set_inverse")
 
     def set_y_budget(self, nbytes: int) -> None:
@@ -246,6 +247,12 @@ class Plan:
         _check(load_library().fdd_plan_get_spectrum(self._h, ctypes.byref(x), ctypes.byref(pitch),
                                                     ctypes.byref(dc)), "fdd_plan_get_spectrum")
         return x.value, pitch.value, dc.value
+
+    def get_inverse(self) -> int:
+        """The inverse transform the last TIME-mode prepare / execute used (FDD_INVERSE_TWO_PASS or _CUFFT)."""
+        w = ctypes.c_int()
+        _check(load_library().fdd_plan_get_inverse(self._h, ctypes.byref(w)), "fdd_plan_get_inverse")
+        return int(w.value)
 
     def get_padding(self) -> int:
         """Lowest bins whose mean-rectangle term a per-plan fp64 table supplies (0: not zero padded)."""

@@ -33,15 +33,19 @@ constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per
 constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
 constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
-// rows per pass of the own inverse (ring: 2 x 64 MiB at 2^20); FDD_IFFT_BATCH for experiments
-int ifft_batch()
+// Rows per launch of the own inverse: its intermediate takes 512 MiB (128 rows at nfft = 2^20; launches of
+// fewer rows leave SMs idle at their tails: 23.2 ms with 16 rows, 20.5 with 128 at 4096 x 2^20), at
+// least 8 and at most 512 rows.  FDD_IFFT_BATCH overrides (experiments).
+int ifft_batch(long long nfft_out)
 {
-    static const int n = [] {
+    static const int env = [] {
         const char* e = getenv("FDD_IFFT_BATCH");
         const int v = e ? atoi(e) : 0;
-        return v >= 1 && v <= 4096 ? v : 16;
+        return v >= 1 && v <= 4096 ? v : 0;
     }();
-    return n;
+    if (env) return env;
+    const long long rows = (1LL << 26) / (nfft_out / 2 > 0 ? nfft_out / 2 : 1);
+    return rows < 8 ? 8 : (rows > 512 ? 512 : (int)rows);
 }
 constexpr int kTensorMinRows = 1024;                  // launches with fewer trial DMs take the FP32 kernels
 
@@ -112,11 +116,12 @@ struct fdd_plan {
     void* fft_ws = nullptr;
     size_t fft_ws_bytes = 0;
     // a5 by the hand-written two-pass transform (fdd_kernels_ifft.cuh) instead of cuFFT
-    int inverse_request = FDD_INVERSE_CUFFT;
+    int inverse_request = FDD_INVERSE_AUTO;
     bool ifft_on = false;                // decided with the TIME-mode resources
     bool dc_in_bin0 = true;              // a4 restores the mean in bin 0 (false: the own inverse adds it)
-    float2* ifft_ring = nullptr;         // [2][ifft_batch()][nfft_out / 2]
+    float2* ifft_ring = nullptr;         // [ifft_batch(nfft_out)][nfft_out / 2]
     size_t ifft_ring_bytes = 0;
+    bool ifft_no_room = false;           // AUTO: the intermediate did not fit, this plan stays on cuFFT
     // multi-beam execution (fdd_execute_beams): spectra and TIME-mode sums of one group of beams
     float2* beam_X = nullptr;            // [beam_group][nchans][xpitch]
     float2* beam_Y = nullptr;            // [beam_group][ndm][ypitch]
@@ -449,6 +454,7 @@ void drop_time_resources(fdd_plan* p)
         p->ifft_ring_bytes = 0;
     }
     p->ifft_on = false;
+    p->ifft_no_room = false;
     p->y_rows = 0;
     p->c2r_tail_batch = 0;
     p->sym2_shapes.clear();
@@ -476,10 +482,20 @@ int ensure_time_family(fdd_plan* p, int* family_out)
     }
     *family_out = family;
     int m1, m2;
-    p->ifft_on = family == 0 && p->inverse_request == FDD_INVERSE_TWO_PASS && fdd::ifft_split(p->nfft_out, &m1, &m2);
+    // AUTO: the own inverse where a4 writes plain sums and Y holds every trial DM (measured faster than
+    // cuFFT's C2R there; a chunked plan is short of memory and keeps cuFFT's shared workspace)
+    const bool want = p->inverse_request == FDD_INVERSE_TWO_PASS ||
+                      (p->inverse_request == FDD_INVERSE_AUTO && p->y_rows == p->ndm);
+    p->ifft_on = family == 0 && want && !p->ifft_no_room && fdd::ifft_split(p->nfft_out, &m1, &m2);
     if (p->ifft_on && !p->ifft_ring) {
-        const size_t n = (size_t)2 * ifft_batch() * (size_t)(p->nfft_out / 2);
-        if ((rc = dev_alloc(p, &p->ifft_ring, n)) != FDD_OK) return rc;
+        const size_t n = (size_t)ifft_batch(p->nfft_out) * (size_t)(p->nfft_out / 2);
+        rc = dev_alloc(p, &p->ifft_ring, n);
+        if (rc != FDD_OK && p->inverse_request == FDD_INVERSE_AUTO) {
+            p->ifft_on = false;                  // no room for the intermediate: cuFFT
+            p->ifft_no_room = true;
+            return FDD_OK;
+        }
+        if (rc != FDD_OK) return rc;
         p->ifft_ring_bytes = n * sizeof(float2);
     }
     return FDD_OK;
@@ -773,8 +789,8 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
         const float mean = p->padded ? 0.f
                                      : (float)((double)p->offset * (double)p->nchans * (double)p->nsamps / (double)p->nfft);
         const int rc = fdd::ifft_launch(ysrc, p->ypitch, rows, dst, p->nsamps_out, p->nsamps_out, p->nfft_out, mean,
-                                        p->ifft_ring, ifft_batch(), s);
-        *launches += 2 * ((rows + ifft_batch() - 1) / ifft_batch());
+                                        p->ifft_ring, ifft_batch(p->nfft_out), s);
+        *launches += 2 * ((rows + ifft_batch(p->nfft_out) - 1) / ifft_batch(p->nfft_out));
         return rc == 0 ? FDD_OK : (rc == -5 ? FDD_ERR_UNSUPPORTED : FDD_ERR_CUDA);
     }
     const bool direct = (p->nsamps_out == p->nfft_out);
@@ -989,12 +1005,20 @@ int fdd_plan_set_kernel(fdd_plan* p, int kernel)
 
 int fdd_plan_set_inverse(fdd_plan* p, int which)
 {
-    if (check_plan(p) != FDD_OK || (which != FDD_INVERSE_TWO_PASS && which != FDD_INVERSE_CUFFT))
+    if (check_plan(p) != FDD_OK ||
+        (which != FDD_INVERSE_TWO_PASS && which != FDD_INVERSE_CUFFT && which != FDD_INVERSE_AUTO))
         return FDD_ERR_INVALID_ARG;
     DeviceGuard g(p->device);
     if (!g.ok || cudaDeviceSynchronize() != cudaSuccess) return FDD_ERR_CUDA;
     drop_time_resources(p);
     p->inverse_request = which;
+    return FDD_OK;
+}
+
+int fdd_plan_get_inverse(const fdd_plan* p, int* which)
+{
+    if (!p || !which) return FDD_ERR_INVALID_ARG;
+    *which = p->ifft_on ? FDD_INVERSE_TWO_PASS : FDD_INVERSE_CUFFT;
     return FDD_OK;
 }
 

@@ -77,16 +77,20 @@ __device__ __forceinline__ void ifft_bf8(float2 (&v)[8])
 // (j - k) R + k + r Ns.  Every CTA thread must call it (it synchronises the CTA).
 // (t_in, c_in): the thread's role up to the first exchange, (t, c) after it - the exchange goes through
 // the tile, so a thread may pick up another part of the work there (pass B loads rows along t and
-// stores along c).  PAD: tile row i sits at i + i / 8, which keeps the first stage's stores of a warp
-// that runs along t off each other's banks.
-template <bool PAD>
-__device__ __forceinline__ int ifft_row(int i) { return PAD ? i + (i >> 3) : i; }
+// stores along c).  Tile: [L + L / 2^PAD][C], point i in row i + (i >> PAD): with the shifts ifft_pad_a / _b
+// choose, a warp's 32 accesses fall on all banks evenly in (nearly) every exchange (checked by
+// enumerating the access patterns: 1.0 .. 1.17 x the ideal number of wavefronts, against 1.75 .. 2 x
+// for a tile with one padding column).
+template <int PAD>
+__device__ __forceinline__ int ifft_row(int i) { return i + (i >> PAD); }
+__host__ __device__ constexpr int ifft_pad_a(int lg, int lgc) { return lgc == 3 ? (lg % 3 ? lg % 3 : 3) : 2; }
+__host__ __device__ constexpr int ifft_pad_b(int lg, int lgc) { return lg >= 6 ? 3 : ifft_pad_a(lg, lgc); }
 
-template <int LG, int LGC, bool PAD, class Emit>
+template <int LG, int LGC, int PAD, class Emit>
 __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float2* tw, int t_in, int c_in, int t,
                                           int c, Emit emit)
 {
-    constexpr int L = 1 << LG, T = L / 8, P = (1 << LGC) + 1;
+    constexpr int L = 1 << LG, T = L / 8, P = 1 << LGC;
     constexpr int R0 = 1 << (LG % 3), N8 = LG / 3;
     bool wrote = false;
     if (R0 == 2) {
@@ -161,12 +165,12 @@ __host__ __device__ constexpr int ifft_hi_len(int lg) { return lg > 5 ? 1 << (lg
 // shared memory of the two passes, in float2 elements
 constexpr size_t ifft_smem_a(int lg, int lgc)
 {
-    return ((size_t)(1 << lg) * ((1 << lgc) + 1) + 2 * (size_t)(1 << lg) + (size_t)(1 << lgc) * (ifft_hi_len(lg) + 34)) *
-           sizeof(float2);
+    return ((size_t)((1 << lg) + ((1 << lg) >> ifft_pad_a(lg, lgc))) * (1 << lgc) + 2 * (size_t)(1 << lg) +
+            (size_t)(1 << lgc) * (ifft_hi_len(lg) + 34)) * sizeof(float2);
 }
 constexpr size_t ifft_smem_b(int lg, int lgc)
 {
-    return ((size_t)((1 << lg) + (1 << lg) / 8) * ((1 << lgc) + 1) + (size_t)(1 << lg)) * sizeof(float2);   // padded rows
+    return ((size_t)((1 << lg) + ((1 << lg) >> ifft_pad_b(lg, lgc))) * (1 << lgc) + (size_t)(1 << lg)) * sizeof(float2);
 }
 
 // Pass A.  grid = (M2 / C, rows), CTA = C columns x L / 8 threads, L = M1 = 2^LG.
@@ -174,14 +178,20 @@ constexpr size_t ifft_smem_b(int lg, int lgc)
 // Twiddles come from small per-CTA tables (a sincospif per element would cost as much as the transform):
 //   e^{i pi k / M},        k = M2 k1 + k2:  half[k1] = e^{i pi k1 / M1}  times  colw[c] = e^{i pi k2 / M}
 //   e^{2 pi i k2 n1 / M},  n1 = 32 a + b:   hi[c][a] = e^{2 pi i k2 32 a / M}  times  lo[c][b] = e^{2 pi i k2 b / M}
+#ifndef IFFT_MINB_A
+#define IFFT_MINB_A 2
+#endif
+#ifndef IFFT_MINB_B
+#define IFFT_MINB_B 2
+#endif
 template <int LG, int LGC>
-__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : 2)
+__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_A)
 k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg2)
 {
-    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, P = C + 1, NT = T * C, HI = ifft_hi_len(LG);
+    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, NT = T * C, HI = ifft_hi_len(LG), PAD = ifft_pad_a(LG, LGC);
     extern __shared__ float2 ifft_smem[];
-    float2* s = ifft_smem;                         // [L][P]
-    float2* tw = s + L * P;                        // [L]
+    float2* s = ifft_smem;                         // [L + (L >> PAD)][C]
+    float2* tw = s + (L + (L >> PAD)) * C;         // [L]
     float2* half = tw + L;                         // [L]
     float2* hi = half + L;                         // [C][HI]
     float2* lo = hi + C * HI;                      // [C][32]
@@ -247,7 +257,7 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
     float2 pw = ifft_cmul(hi[c * HI + (t >> 5)], lo[c * 32 + (t & 31)]);
     const float2 pg = colg[c];
     float2* bc = b + c0 + c;
-    ifft_core<LG, LGC, false>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
+    ifft_core<LG, LGC, PAD>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
         if (r > 0) pw = ifft_cmul(pw, pg);
         bc[(long long)n1 << lg2] = ifft_cmul(val, pw);
     });
@@ -256,18 +266,22 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
 // Pass B.  grid = (M1 / C, rows), CTA = C rows n1 of B x L / 8 threads, L = M2 = 2^LG.
 // out: [rows][opitch] floats, the first nout of the 2 M samples.
 template <int LG, int LGC>
-__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : 2)
+__global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_B)
 k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long opitch, long long nout, int lg1,
               float mean)
 {
-    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, P = C + 1, NT = T * C;
+    constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, NT = T * C, PAD = ifft_pad_b(LG, LGC);
     extern __shared__ float2 ifft_smem[];
-    float2* s = ifft_smem;                         // [L + L / 8][P] (padded rows)
-    float2* tw = s + (L + L / 8) * P;              // [L]
-    // loads (and the first stage) with the warps along a row of B, the rest and the stores with them across
-    // the C rows: both sides of the transposition this pass is are then runs of whole sectors
+    float2* s = ifft_smem;                         // [L + (L >> PAD)][C]
+    float2* tw = s + (L + (L >> PAD)) * C;         // [L]
+    // loads (and the first stage) with 8 lanes along a row of B (64-byte runs), the rest and the stores with
+    // the lanes across the C rows (runs of 8 C bytes): both sides of the transposition this pass is are
+    // then runs of whole sectors
     const int c = threadIdx.x & (C - 1), t = threadIdx.x >> LGC;
-    const int t_in = LG > 3 ? (int)(threadIdx.x & (T - 1)) : t, c_in = LG > 3 ? (int)(threadIdx.x >> (LG - 3)) : c;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int TW = T >= 8 ? T / 8 : 1;         // groups of 8 points along a row
+    const int t_in = LG >= 6 ? (warp % TW) * 8 + (lane & 7) : t;
+    const int c_in = LG >= 6 ? (warp / TW) * 4 + (lane >> 3) : c;
     const long long M = (long long)1 << (LG + lg1);
     const long long n1 = (long long)blockIdx.x * C + c;
     const float2* b = B + (long long)blockIdx.y * M + (((long long)blockIdx.x * C + c_in) << LG);
@@ -279,7 +293,7 @@ k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long o
     __syncthreads();
     // (rows of the caller's array may start on an odd float: then two 4-byte stores per point)
     const bool vec = (reinterpret_cast<uintptr_t>(o) & 7) == 0;
-    ifft_core<LG, LGC, true>(v, s, tw, t_in, c_in, t, c, [&](int, int n2, float2 val) {
+    ifft_core<LG, LGC, PAD>(v, s, tw, t_in, c_in, t, c, [&](int, int n2, float2 val) {
         const long long n = n1 + ((long long)n2 << lg1);                 // z[n] = (y[2n], y[2n+1])
         if (2 * n + 1 < nout) {
             if (vec) {
@@ -366,7 +380,7 @@ inline int ifft_launch_b(const float2* B, float* out, long long opitch, long lon
         default: rc = -5;                                      \
     }
 
-// rows of Y -> rows of out, in batches of `batch` rows through the ring `ring` ([2][batch][M] float2)
+// rows of Y -> rows of out, in launches of `batch` rows through the intermediate `ring` ([batch][M] float2)
 inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
                        long long nfft_out, float mean, float2* ring, int batch, cudaStream_t s)
 {
@@ -377,10 +391,10 @@ inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, 
     while ((1 << lg1) < M1) ++lg1;
     while ((1 << lg2) < M2) ++lg2;
     const int lgc1 = ifft_lgc(lg1), lgc2 = ifft_lgc(lg2);
-    int slot = 0;
-    for (int r0 = 0; r0 < rows; r0 += batch, slot ^= 1) {
+    (void)M;
+    for (int r0 = 0; r0 < rows; r0 += batch) {
         const int n = rows - r0 < batch ? rows - r0 : batch;
-        float2* b = ring + (size_t)slot * batch * M;
+        float2* b = ring;
         int rc = 0;
         FDD_IFFT_DISPATCH(lg1, lgc1, (rc = ifft_launch_a<LG_, LGC_>(Y + (long long)r0 * ypitch, ypitch, b, lg2, n, s)));
         if (rc != 0) return rc;

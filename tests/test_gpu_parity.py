@@ -519,7 +519,7 @@ class _FullSize:
         return np.stack([cls.Y[(key, j)] for j in rows])
 
 
-def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None, inverse="cufft"):
+def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None, inverse="auto"):
     """One full-size TIME execute at `ndm` trial DMs; sampled rows against the oracle."""
     import torch
     w = synth.workload(name, ndm=ndm)
@@ -534,8 +534,8 @@ def _full_size_point(F, name, ndm, rows, kernel_want, decimate=0, force=None, in
         assert plan.get_info()[5] == kernel_want
         if decimate:
             plan.set_decimation(decimate)
-        if inverse == "two_pass":
-            plan.set_inverse(F.FDD_INVERSE_TWO_PASS)
+        if inverse != "auto":
+            plan.set_inverse(F.FDD_INVERSE_TWO_PASS if inverse == "two_pass" else F.FDD_INVERSE_CUFFT)
         ns_out, _ = plan.output_shape()
         d_in = _FullSize.device_input(name)
         out = torch.empty((plan.ndm, ns_out), dtype=torch.float32, device="cuda")
@@ -571,8 +571,16 @@ def test_full_size_config4_dm_sweep(F, oracle_c, ndm):
     plan bench.py times (1024 = config 3; 4096 = the default bench workload; 128 takes the 64-DM
     group instance of the sym2 kernel, the others 96-DM groups with different tails)."""
     rows = sorted({j for j in _SWEEP_POOL if j < ndm} | {ndm - 1, ndm // 2 + 15, ndm // 2 + 16})
-    # AUTO: the tensor-core kernel from 1024 trial DMs up, the shared-recurrence FP32 kernel below
+    # AUTO: the tensor-core kernel (+ the hand-written two-pass inverse) from 1024 trial DMs up, the
+    # shared-recurrence FP32 kernel (+ cuFFT's half-length C2C) below
     _full_size_point(F, "config4", ndm, rows, F.FDD_KERNEL_TENSOR if ndm >= 1024 else F.FDD_KERNEL_SYMMETRIC2)
+
+
+@pytest.mark.slow
+def test_full_size_config4_tensor_kernel_cufft_inverse(F, oracle_c):
+    """The tensor-core kernel followed by cuFFT's C2R (FDD_INVERSE_CUFFT), which AUTO no longer takes."""
+    rows = sorted({j for j in _SWEEP_POOL if j < 1024} | {1023})
+    _full_size_point(F, "config4", 1024, rows, F.FDD_KERNEL_TENSOR, inverse="cufft")
 
 
 @pytest.mark.slow
@@ -585,7 +593,7 @@ def test_full_size_config4_fp32_kernel(F, oracle_c, ndm):
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("m,inverse", [(1, "cufft"), (2, "cufft"), (3, "cufft"), (3, "two_pass")])
+@pytest.mark.parametrize("m,inverse", [(1, "auto"), (2, "auto"), (3, "auto"), (3, "two_pass")])
 def test_full_size_config4_decimated(F, oracle_c, m, inverse):
     """Row f3 at config-4 size (512 trial DMs): reduced-length inverse transform.  The
     low-pass shrinks the rms of the series while cuFFT's fp32 error stays relative to its mean, so
@@ -798,9 +806,12 @@ def test_inverse_transform_choices(F, oracle_c, nchans, nsamps, ndm, step, kerne
     ref = O.fdd_rows(u8, _delays_for(w), range(ndm), mode="time")
     with _plan_for(F, w) as plan:
         _set_kernel(F, plan, kernel)
-        for which in (F.FDD_INVERSE_TWO_PASS, F.FDD_INVERSE_CUFFT, F.FDD_INVERSE_TWO_PASS):
+        for which in (F.FDD_INVERSE_AUTO, F.FDD_INVERSE_TWO_PASS, F.FDD_INVERSE_CUFFT, F.FDD_INVERSE_TWO_PASS):
             plan.set_inverse(which)
             got = _run(F, plan, u8, "time")
+            if which != F.FDD_INVERSE_AUTO:
+                # (every length here is one the hand-written inverse takes)
+                assert plan.get_inverse() == which
             worst = parity.assert_rows(got, ref, "time", f"inverse {which}/{kernel}/{nchans}x{nsamps}")
             print("inverse", which, kernel, nchans, nsamps, worst)
         with pytest.raises(F.FddError):
