@@ -96,8 +96,8 @@ enum fdd_inverse {
                                   2^20, 57 vs 82 ms at 1024 x 2^23), slower than the C2C behind
                                   SYMMETRIC2's fused pre-twiddle; cuFFT for other lengths              */
     FDD_INVERSE_AUTO = 2       /* the default: TWO_PASS where it applies, a4 writes plain sums (every a4
-                                  kernel but SYMMETRIC2) and the sums of all trial DMs fit the plan's Y
-                                  scratch at once; CUFFT otherwise                                     */
+                                  kernel but SYMMETRIC2) and its 512 MiB intermediate fits; CUFFT
+                                  otherwise                                                            */
 };
 
 /* Stage indices for fdd_plan_get_stage_ms. */

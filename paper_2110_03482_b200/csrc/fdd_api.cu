@@ -121,6 +121,8 @@ struct fdd_plan {
     bool dc_in_bin0 = true;              // a4 restores the mean in bin 0 (false: the own inverse adds it)
     float2* ifft_ring = nullptr;         // [ifft_batch(nfft_out)][nfft_out / 2]
     size_t ifft_ring_bytes = 0;
+    float2* ifft_tab = nullptr;          // the own inverse's twiddle tables (fdd_kernels_ifft.cuh)
+    size_t ifft_tab_bytes = 0;
     bool ifft_no_room = false;           // AUTO: the intermediate did not fit, this plan stays on cuFFT
     // multi-beam execution (fdd_execute_beams): spectra and TIME-mode sums of one group of beams
     float2* beam_X = nullptr;            // [beam_group][nchans][xpitch]
@@ -453,6 +455,12 @@ void drop_time_resources(fdd_plan* p)
         p->ifft_ring = nullptr;
         p->ifft_ring_bytes = 0;
     }
+    if (p->ifft_tab) {
+        cudaFree(p->ifft_tab);
+        p->scratch_bytes -= p->ifft_tab_bytes;
+        p->ifft_tab = nullptr;
+        p->ifft_tab_bytes = 0;
+    }
     p->ifft_on = false;
     p->ifft_no_room = false;
     p->y_rows = 0;
@@ -482,10 +490,9 @@ int ensure_time_family(fdd_plan* p, int* family_out)
     }
     *family_out = family;
     int m1, m2;
-    // AUTO: the own inverse where a4 writes plain sums and Y holds every trial DM (measured faster than
-    // cuFFT's C2R there; a chunked plan is short of memory and keeps cuFFT's shared workspace)
-    const bool want = p->inverse_request == FDD_INVERSE_TWO_PASS ||
-                      (p->inverse_request == FDD_INVERSE_AUTO && p->y_rows == p->ndm);
+    // AUTO: the own inverse where a4 writes plain sums (measured faster than cuFFT's C2R there), unless
+    // its intermediate does not fit
+    const bool want = p->inverse_request == FDD_INVERSE_TWO_PASS || p->inverse_request == FDD_INVERSE_AUTO;
     p->ifft_on = family == 0 && want && !p->ifft_no_room && fdd::ifft_split(p->nfft_out, &m1, &m2);
     if (p->ifft_on && !p->ifft_ring) {
         const size_t n = (size_t)ifft_batch(p->nfft_out) * (size_t)(p->nfft_out / 2);
@@ -497,6 +504,19 @@ int ensure_time_family(fdd_plan* p, int* family_out)
         }
         if (rc != FDD_OK) return rc;
         p->ifft_ring_bytes = n * sizeof(float2);
+    }
+    if (p->ifft_on && !p->ifft_tab) {
+        int l1 = 0, l2 = 0;
+        while ((1 << l1) < m1) ++l1;
+        while ((1 << l2) < m2) ++l2;
+        const size_t n = fdd::ifft_table_elems(l1, l2);
+        if ((rc = dev_alloc(p, &p->ifft_tab, n)) != FDD_OK) return rc;
+        p->ifft_tab_bytes = n * sizeof(float2);
+        // (made on the default stream; synchronised so that an execute on any stream finds it)
+        if (fdd::ifft_make_tables(p->nfft_out, p->ifft_tab, nullptr) != 0 || cudaDeviceSynchronize() != cudaSuccess) {
+            cudaGetLastError();
+            return FDD_ERR_CUDA;
+        }
     }
     return FDD_OK;
 }
@@ -524,6 +544,7 @@ void destroy_plan(fdd_plan* p)
     cudaFree(p->stage_out);
     cudaFree(p->pad_tab);
     cudaFree(p->ifft_ring);
+    cudaFree(p->ifft_tab);
     cudaFree(p->beam_X);
     cudaFree(p->beam_Y);
     fdd::sym_free_tables(&p->sym);
@@ -789,7 +810,7 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
         const float mean = p->padded ? 0.f
                                      : (float)((double)p->offset * (double)p->nchans * (double)p->nsamps / (double)p->nfft);
         const int rc = fdd::ifft_launch(ysrc, p->ypitch, rows, dst, p->nsamps_out, p->nsamps_out, p->nfft_out, mean,
-                                        p->ifft_ring, ifft_batch(p->nfft_out), s);
+                                        p->ifft_ring, p->ifft_tab, ifft_batch(p->nfft_out), s);
         *launches += 2 * ((rows + ifft_batch(p->nfft_out) - 1) / ifft_batch(p->nfft_out));
         return rc == 0 ? FDD_OK : (rc == -5 ? FDD_ERR_UNSUPPORTED : FDD_ERR_CUDA);
     }

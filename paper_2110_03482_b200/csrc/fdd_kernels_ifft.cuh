@@ -33,8 +33,9 @@ __device__ __forceinline__ float2 ifft_cmul(float2 a, float2 b)
 {
     return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
-__device__ __forceinline__ float2 ifft_add(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 ifft_sub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// (packed fp32 pairs: one FADD2 per complex sum)
+__device__ __forceinline__ float2 ifft_add(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 ifft_sub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
 
 // Butterflies with the kernel e^{+2 pi i p q / R}, in place, outputs in natural order
 __device__ __forceinline__ void ifft_bf2(float2& a, float2& b)
@@ -86,6 +87,14 @@ __device__ __forceinline__ int ifft_row(int i) { return i + (i >> PAD); }
 __host__ __device__ constexpr int ifft_pad_a(int lg, int lgc) { return lgc == 3 ? (lg % 3 ? lg % 3 : 3) : 2; }
 __host__ __device__ constexpr int ifft_pad_b(int lg, int lgc) { return lg >= 6 ? 3 : ifft_pad_a(lg, lgc); }
 
+// row of point i0 + d, d a compile-time multiple: where the padding is linear in d (d a multiple of 2^PAD, or
+// i0 a multiple of 2^PAD and d below it) the offset is a constant the compiler folds into the access
+template <int PAD>
+__device__ __forceinline__ int ifft_row_at(int row_i0, int i0, int d, bool linear)
+{
+    return linear ? row_i0 + d + (d >> PAD) : ifft_row<PAD>(i0 + d);
+}
+
 template <int LG, int LGC, int PAD, class Emit>
 __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float2* tw, int t_in, int c_in, int t,
                                           int c, Emit emit)
@@ -115,8 +124,11 @@ __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float
     }
     if (wrote) {
         __syncthreads();
+        {
+            const int rt = ifft_row<PAD>(t);
 #pragma unroll
-        for (int q = 0; q < 8; ++q) v[q] = s[ifft_row<PAD>(t + q * T) * P + c];
+            for (int q = 0; q < 8; ++q) v[q] = s[ifft_row_at<PAD>(rt, t, q * T, T % (1 << PAD) == 0) * P + c];
+        }
     }
 #pragma unroll
     for (int i = 0; i < N8; ++i) {
@@ -140,12 +152,20 @@ __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float
             for (int r = 0; r < 8; ++r) emit(r, j0 + r * Ns, v[r]);
         } else {
             if (wrote) __syncthreads();              // the reads of the stage before are done
+            {
+                // (Ns a multiple of 2^PAD: linear; Ns = 1 with 2^PAD >= 8: j0 = 8 t is a multiple of 8 and r < 8)
+                const int rj = ifft_row<PAD>(j0);
+                const bool lin = Ns % (1 << PAD) == 0 || (Ns == 1 && PAD >= 3);
 #pragma unroll
-            for (int r = 0; r < 8; ++r) s[ifft_row<PAD>(j0 + r * Ns) * P + cc] = v[r];
+                for (int r = 0; r < 8; ++r) s[ifft_row_at<PAD>(rj, j0, r * Ns, lin) * P + cc] = v[r];
+            }
             wrote = true;
             __syncthreads();
+            {
+                const int rt = ifft_row<PAD>(t);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = s[ifft_row<PAD>(t + q * T) * P + c];
+                for (int q = 0; q < 8; ++q) v[q] = s[ifft_row_at<PAD>(rt, t, q * T, T % (1 << PAD) == 0) * P + c];
+            }
         }
     }
 }
@@ -173,6 +193,40 @@ constexpr size_t ifft_smem_b(int lg, int lgc)
     return ((size_t)((1 << lg) + ((1 << lg) >> ifft_pad_b(lg, lgc))) * (1 << lgc) + (size_t)(1 << lg)) * sizeof(float2);
 }
 
+// Per-plan twiddle tables (a sincospif per CTA thread and table entry costs 13 % of the passes'
+// instructions): [tw1: L1][half: L1][tw2: L2][per column k2 < M2: hi (HI), lo (32), colw, colg], float2.
+//   tw[j]   = e^{2 pi i j / L}          half[j] = e^{i pi j / L1}
+//   e^{i pi k / M},        k = M2 k1 + k2:  half[k1] times colw[k2] = e^{i pi k2 / M}
+//   e^{2 pi i k2 n1 / M},  n1 = 32 a + b:   hi[k2][a] = e^{2 pi i k2 32 a / M} times lo[k2][b] = e^{2 pi i k2 b / M};
+//                                           colg[k2] = e^{2 pi i k2 (L1 / 8) / M} steps n1 by L1 / 8
+inline size_t ifft_table_elems(int lg1, int lg2)
+{
+    return 2 * ((size_t)1 << lg1) + ((size_t)1 << lg2) + ((size_t)1 << lg2) * (ifft_hi_len(lg1) + 34);
+}
+
+__global__ void __launch_bounds__(256) k_ifft_tables(float2* tab, int lg1, int lg2)
+{
+    const long long L1 = 1LL << lg1, L2 = 1LL << lg2, M = L1 * L2;
+    const int HI = lg1 > 5 ? 1 << (lg1 - 5) : 1, W = HI + 34;
+    const long long n = 2 * L1 + L2 + L2 * W;
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    double arg;                                     // in half turns (sincospi)
+    if (i < L1) arg = 2.0 * (double)i / (double)L1;
+    else if (i < 2 * L1) arg = (double)(i - L1) / (double)L1;
+    else if (i < 2 * L1 + L2) arg = 2.0 * (double)(i - 2 * L1) / (double)L2;
+    else {
+        const long long e = i - 2 * L1 - L2, k2 = e / W, r = e - k2 * W;
+        if (r < HI) arg = 2.0 * (double)((k2 * 32 * r) % M) / (double)M;
+        else if (r < HI + 32) arg = 2.0 * (double)(k2 * (r - HI)) / (double)M;
+        else if (r == HI + 32) arg = (double)k2 / (double)M;
+        else arg = 2.0 * (double)((k2 * (L1 / 8)) % M) / (double)M;
+    }
+    double sn, cs;
+    sincospi(arg, &sn, &cs);
+    tab[i] = make_float2((float)cs, (float)sn);
+}
+
 // Pass A.  grid = (M2 / C, rows), CTA = C columns x L / 8 threads, L = M1 = 2^LG.
 // Y: [rows][ypitch] sums of a4 (bins 0 .. M); B: [rows][M] as [n1][k2].
 // Twiddles come from small per-CTA tables (a sincospif per element would cost as much as the transform):
@@ -186,23 +240,31 @@ constexpr size_t ifft_smem_b(int lg, int lgc)
 #endif
 template <int LG, int LGC>
 __global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_A)
-k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg2)
+k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg2,
+              const float2* __restrict__ tab)
 {
     constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, NT = T * C, HI = ifft_hi_len(LG), PAD = ifft_pad_a(LG, LGC);
-    extern __shared__ float2 ifft_smem[];
+    extern __shared__ __align__(16) float2 ifft_smem[];
     float2* s = ifft_smem;                         // [L + (L >> PAD)][C]
     float2* tw = s + (L + (L >> PAD)) * C;         // [L]
     float2* half = tw + L;                         // [L]
-    float2* hi = half + L;                         // [C][HI]
-    float2* lo = hi + C * HI;                      // [C][32]
-    float2* colw = lo + C * 32;                    // [C] e^{i pi k2 / M}
-    float2* colg = colw + C;                       // [C] e^{2 pi i k2 (L / 8) / M}
+    float2* colt = half + L;                       // [C][W]: hi (HI), lo (32), colw, colg of each column
+    constexpr int W = HI + 34;
     const int c = threadIdx.x & (C - 1), t = threadIdx.x >> LGC;
     const long long M = (long long)1 << (LG + lg2);
     const float2* y = Y + (long long)blockIdx.y * ypitch;
     float2* b = B + (long long)blockIdx.y * M;
     const int c0 = blockIdx.x * C;
-    // the loads first: they are in flight while the tables are made
+    // tables first (tw and half are the first 2 L entries of the plan's table, this CTA's columns one run
+    // of it: two straight copies, 16 bytes per lane), then the data: the tables land while the data fly
+    {
+        const float4* g = reinterpret_cast<const float4*>(tab);
+        float4* d = reinterpret_cast<float4*>(tw);
+        for (int j = threadIdx.x; j < L; j += NT) d[j] = __ldg(g + j);
+        const float4* gc = reinterpret_cast<const float4*>(tab + 2 * L + ((size_t)1 << lg2) + (size_t)c0 * W);
+        float4* dc = reinterpret_cast<float4*>(colt);
+        for (int j = threadIdx.x; j < C * W / 2; j += NT) dc[j] = __ldg(gc + j);
+    }
     float2 v[8], m[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
@@ -210,35 +272,9 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
         v[q] = y[k];
         m[q] = y[M - k];
     }
-    ifft_make_twiddles(tw, L, NT);
-    const float inv_m = 1.f / (float)M;
-    for (int j = threadIdx.x; j < L; j += NT) {
-        float sn, cs;
-        sincospif((float)j / (float)L, &sn, &cs);
-        half[j] = make_float2(cs, sn);
-    }
-    for (int j = threadIdx.x; j < C * (HI + 32); j += NT) {
-        const int cc = j / (HI + 32), r = j - cc * (HI + 32);
-        const long long k2 = c0 + cc;
-        float sn, cs;
-        if (r < HI) {                              // exact arguments: k2 * 32 a < M2 * M1 = M <= 2^22
-            sincospif(2.f * (float)(k2 * 32 * r) * inv_m, &sn, &cs);
-            hi[cc * HI + r] = make_float2(cs, sn);
-        } else {
-            sincospif(2.f * (float)(k2 * (r - HI)) * inv_m, &sn, &cs);
-            lo[cc * 32 + (r - HI)] = make_float2(cs, sn);
-        }
-    }
-    if (threadIdx.x < C) {
-        float sn, cs;
-        sincospif((float)(c0 + threadIdx.x) * inv_m, &sn, &cs);
-        colw[threadIdx.x] = make_float2(cs, sn);
-        sincospif(2.f * (float)((long long)(c0 + threadIdx.x) * T) * inv_m, &sn, &cs);
-        colg[threadIdx.x] = make_float2(cs, sn);
-    }
     __syncthreads();
     // e^{+2 pi i k / N} = e^{i pi k1 / M1} e^{i pi k2 / M}, k1 = t + q L / 8: half[t] colw[c] times e^{i pi q / 8}
-    const float2 w0 = ifft_cmul(half[t], colw[c]);
+    const float2 w0 = ifft_cmul(half[t], colt[c * W + HI + 32]);
     const float kc[8] = {1.f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f,
                          0.f, -0.38268343236508977f, -0.70710678118654752f, -0.92387953251128674f};
     const float ks[8] = {0.f, 0.38268343236508977f, 0.70710678118654752f, 0.92387953251128674f,
@@ -254,8 +290,8 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
     }
     // e^{+2 pi i k2 n1 / M} for the outputs n1 = t + r L / 8 in turn: the first from the hi / lo tables, then
     // times colg[c] each
-    float2 pw = ifft_cmul(hi[c * HI + (t >> 5)], lo[c * 32 + (t & 31)]);
-    const float2 pg = colg[c];
+    float2 pw = ifft_cmul(colt[c * W + (t >> 5)], colt[c * W + HI + (t & 31)]);
+    const float2 pg = colt[c * W + HI + 33];
     float2* bc = b + c0 + c;
     ifft_core<LG, LGC, PAD>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
         if (r > 0) pw = ifft_cmul(pw, pg);
@@ -268,10 +304,10 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
 template <int LG, int LGC>
 __global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_B)
 k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long opitch, long long nout, int lg1,
-              float mean)
+              float mean, const float2* __restrict__ tab)
 {
     constexpr int L = 1 << LG, C = 1 << LGC, T = L / 8, NT = T * C, PAD = ifft_pad_b(LG, LGC);
-    extern __shared__ float2 ifft_smem[];
+    extern __shared__ __align__(16) float2 ifft_smem[];
     float2* s = ifft_smem;                         // [L + (L >> PAD)][C]
     float2* tw = s + (L + (L >> PAD)) * C;         // [L]
     // loads (and the first stage) with 8 lanes along a row of B (64-byte runs), the rest and the stores with
@@ -286,10 +322,14 @@ k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long o
     const long long n1 = (long long)blockIdx.x * C + c;
     const float2* b = B + (long long)blockIdx.y * M + (((long long)blockIdx.x * C + c_in) << LG);
     float* o = out + (long long)blockIdx.y * opitch;
+    {
+        const float4* g = reinterpret_cast<const float4*>(tab + ((size_t)2 << lg1));
+        float4* d = reinterpret_cast<float4*>(tw);
+        for (int j = threadIdx.x; j < L / 2; j += NT) d[j] = __ldg(g + j);
+    }
     float2 v[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) v[q] = b[t_in + q * T];
-    ifft_make_twiddles(tw, L, NT);
     __syncthreads();
     // (rows of the caller's array may start on an odd float: then two 4-byte stores per point)
     const bool vec = (reinterpret_cast<uintptr_t>(o) & 7) == 0;
@@ -333,7 +373,8 @@ inline int ifft_lgc(int lg)
 }
 
 template <int LG, int LGC>
-inline int ifft_launch_a(const float2* Y, long long ypitch, float2* B, int lg2, int rows, cudaStream_t s)
+inline int ifft_launch_a(const float2* Y, long long ypitch, float2* B, int lg2, const float2* tab, int rows,
+                         cudaStream_t s)
 {
     static bool attr = false;
     constexpr size_t bytes = ifft_smem_a(LG, LGC);
@@ -344,13 +385,13 @@ inline int ifft_launch_a(const float2* Y, long long ypitch, float2* B, int lg2, 
         attr = true;
     }
     k_ifft_pass_a<LG, LGC><<<dim3((unsigned)((1 << lg2) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
-        Y, ypitch, B, lg2);
+        Y, ypitch, B, lg2, tab);
     return 0;
 }
 
 template <int LG, int LGC>
 inline int ifft_launch_b(const float2* B, float* out, long long opitch, long long nout, int lg1, float mean,
-                         int rows, cudaStream_t s)
+                         const float2* tab, int rows, cudaStream_t s)
 {
     static bool attr = false;
     constexpr size_t bytes = ifft_smem_b(LG, LGC);
@@ -361,7 +402,7 @@ inline int ifft_launch_b(const float2* B, float* out, long long opitch, long lon
         attr = true;
     }
     k_ifft_pass_b<LG, LGC><<<dim3((unsigned)((1 << lg1) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
-        B, out, opitch, nout, lg1, mean);
+        B, out, opitch, nout, lg1, mean, tab);
     return 0;
 }
 
@@ -380,9 +421,22 @@ inline int ifft_launch_b(const float2* B, float* out, long long opitch, long lon
         default: rc = -5;                                      \
     }
 
+// the plan's table for nfft_out (ifft_table_elems float2 at tab), made on stream s
+inline int ifft_make_tables(long long nfft_out, float2* tab, cudaStream_t s)
+{
+    int M1, M2;
+    if (!ifft_split(nfft_out, &M1, &M2)) return -5;
+    int lg1 = 0, lg2 = 0;
+    while ((1 << lg1) < M1) ++lg1;
+    while ((1 << lg2) < M2) ++lg2;
+    const size_t n = ifft_table_elems(lg1, lg2);
+    k_ifft_tables<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(tab, lg1, lg2);
+    return cudaGetLastError() == cudaSuccess ? 0 : -3;
+}
+
 // rows of Y -> rows of out, in launches of `batch` rows through the intermediate `ring` ([batch][M] float2)
 inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
-                       long long nfft_out, float mean, float2* ring, int batch, cudaStream_t s)
+                       long long nfft_out, float mean, float2* ring, const float2* tab, int batch, cudaStream_t s)
 {
     int M1, M2;
     if (!ifft_split(nfft_out, &M1, &M2)) return -5;
@@ -396,10 +450,10 @@ inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, 
         const int n = rows - r0 < batch ? rows - r0 : batch;
         float2* b = ring;
         int rc = 0;
-        FDD_IFFT_DISPATCH(lg1, lgc1, (rc = ifft_launch_a<LG_, LGC_>(Y + (long long)r0 * ypitch, ypitch, b, lg2, n, s)));
+        FDD_IFFT_DISPATCH(lg1, lgc1, (rc = ifft_launch_a<LG_, LGC_>(Y + (long long)r0 * ypitch, ypitch, b, lg2, tab, n, s)));
         if (rc != 0) return rc;
         FDD_IFFT_DISPATCH(lg2, lgc2, (rc = ifft_launch_b<LG_, LGC_>(b, out + (long long)r0 * opitch, opitch, nout,
-                                                                     lg1, mean, n, s)));
+                                                                     lg1, mean, tab, n, s)));
         if (rc != 0) return rc;
     }
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
