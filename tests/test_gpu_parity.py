@@ -797,6 +797,13 @@ def test_multi_beam_config3_eight_beams(F, oracle_c):
     (20, 6000, 70, 0.9),             # zero padded, output cropped to 6000 of 8192 samples
     (8, 1 << 17, 33, 2.0),           # M = 2^16 = 256 x 256
     (12, 1001, 9, 0.3),              # odd series length
+    (4, 1 << 14, 9, 1.1),            # M = 2^13 = 64 x 128: every transform length of the two passes once
+    (4, 1 << 15, 9, 1.3),            # M = 2^14 = 128 x 128
+    (4, 1 << 16, 6, 1.7),            # M = 2^15 = 128 x 256
+    (4, 1 << 18, 5, 2.3),            # M = 2^17 = 256 x 512
+    (4, 1 << 19, 5, 3.1),            # M = 2^18 = 512 x 512
+    (3, 1 << 21, 3, 5.0),            # M = 2^20 = 1024 x 1024
+    (2, 1 << 22, 3, 7.0),            # M = 2^21 = 1024 x 2048
 ])
 def test_inverse_transform_choices(F, oracle_c, nchans, nsamps, ndm, step, kernel):
     """FDD_INVERSE_TWO_PASS (the hand-written two-pass inverse, which also restores the mean after the
