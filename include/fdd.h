@@ -92,8 +92,8 @@ enum fdd_inverse {
                                   (radix-8 butterflies in registers): forms the half-length spectrum in
                                   its first pass and adds the series' mean after the transform, so fp32
                                   works on a series of rms sigma instead of 256 sigma (TIME-mode error
-                                  about 2x smaller).  Faster than cuFFT's C2R (20.5 vs 21.1 ms at 4096 x
-                                  2^20, 57 vs 82 ms at 1024 x 2^23), slower than the C2C behind
+                                  about 2x smaller).  Faster than cuFFT's C2R (18.8 vs 21.1 ms at 4096 x
+                                  2^20, 55 vs 82 ms at 1024 x 2^23), slower than the C2C behind
                                   SYMMETRIC2's fused pre-twiddle; cuFFT for other lengths              */
     FDD_INVERSE_AUTO = 2       /* the default: TWO_PASS where it applies, a4 writes plain sums (every a4
                                   kernel but SYMMETRIC2) and its 512 MiB intermediate fits; CUFFT

@@ -810,7 +810,7 @@ int launch_c2r_rows(fdd_plan* p, int family, int rows, float2* ysrc, float* dst,
         const float mean = p->padded ? 0.f
                                      : (float)((double)p->offset * (double)p->nchans * (double)p->nsamps / (double)p->nfft);
         const int rc = fdd::ifft_launch(ysrc, p->ypitch, rows, dst, p->nsamps_out, p->nsamps_out, p->nfft_out, mean,
-                                        p->ifft_ring, p->ifft_tab, ifft_batch(p->nfft_out), s);
+                                        p->ifft_ring, p->ifft_tab, ifft_batch(p->nfft_out), p->padded, s);
         *launches += 2 * ((rows + ifft_batch(p->nfft_out) - 1) / ifft_batch(p->nfft_out));
         return rc == 0 ? FDD_OK : (rc == -5 ? FDD_ERR_UNSUPPORTED : FDD_ERR_CUDA);
     }

@@ -95,7 +95,11 @@ __device__ __forceinline__ int ifft_row_at(int row_i0, int i0, int d, bool linea
     return linear ? row_i0 + d + (d >> PAD) : ifft_row<PAD>(i0 + d);
 }
 
-template <int LG, int LGC, int PAD, class Emit>
+// ACC: every twiddle straight from a table (zero-padded series keep their mean - a rectangle 256 sigma high -
+// inside the transform, and at 2^23 points the products and recurrences that save table loads cost the
+// margin: max error 1.04e-3 of the rms against 0.98e-3; without padding the mean is outside, either passes
+// with a wide margin and the cheaper form is 1.7 ms faster at 4096 x 2^20)
+template <int LG, int LGC, int PAD, bool ACC, class Emit>
 __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float2* tw, int t_in, int c_in, int t,
                                           int c, Emit emit)
 {
@@ -139,8 +143,10 @@ __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float
             // w^r, r = 1 .. 7, w = e^{2 pi i k / (8 Ns)}: three from the table, four products
             const int step = L / (8 * Ns);
             const float2 w1 = tw[k * step], w2 = tw[2 * k * step], w4 = tw[4 * k * step];
-            const float2 w3 = ifft_cmul(w1, w2), w5 = ifft_cmul(w1, w4), w6 = ifft_cmul(w2, w4);
-            const float2 w7 = ifft_cmul(w3, w4);
+            const float2 w3 = ACC ? tw[3 * k * step] : ifft_cmul(w1, w2);
+            const float2 w5 = ACC ? tw[5 * k * step] : ifft_cmul(w1, w4);
+            const float2 w6 = ACC ? tw[6 * k * step] : ifft_cmul(w2, w4);
+            const float2 w7 = ACC ? tw[7 * k * step] : ifft_cmul(w3, w4);
             v[1] = ifft_cmul(v[1], w1); v[2] = ifft_cmul(v[2], w2); v[3] = ifft_cmul(v[3], w3);
             v[4] = ifft_cmul(v[4], w4); v[5] = ifft_cmul(v[5], w5); v[6] = ifft_cmul(v[6], w6);
             v[7] = ifft_cmul(v[7], w7);
@@ -165,6 +171,95 @@ __device__ __forceinline__ void ifft_core(float2 (&v)[8], float2* s, const float
                 const int rt = ifft_row<PAD>(t);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) v[q] = s[ifft_row_at<PAD>(rt, t, q * T, T % (1 << PAD) == 0) * P + c];
+            }
+        }
+    }
+}
+
+// Two transforms per thread (columns 2 c and 2 c + 1 of a tile [rows][2 C], moved as one 16-byte access;
+// one set of twiddles for both): same stages as ifft_core, no change of roles.
+template <int LG, int LGC, int PAD, bool ACC, class Emit>
+__device__ __forceinline__ void ifft_core2(float2 (&va)[8], float2 (&vb)[8], float2* s, const float2* tw, int t, int c,
+                                           Emit emit)
+{
+    constexpr int L = 1 << LG, T = L / 8, P4 = 1 << LGC;       // float4 per tile row
+    constexpr int R0 = 1 << (LG % 3), N8 = LG / 3;
+    float4* s4 = reinterpret_cast<float4*>(s);
+    auto put = [&](int row, float2 a, float2 b) { s4[row * P4 + c] = make_float4(a.x, a.y, b.x, b.y); };
+    auto get = [&](int row, float2& a, float2& b) {
+        const float4 w = s4[row * P4 + c];
+        a = make_float2(w.x, w.y);
+        b = make_float2(w.z, w.w);
+    };
+    bool wrote = false;
+    if (R0 == 2) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            ifft_bf2(va[u], va[u + 4]);
+            ifft_bf2(vb[u], vb[u + 4]);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            put(ifft_row<PAD>(2 * (t + u * T)), va[u], vb[u]);
+            put(ifft_row<PAD>(2 * (t + u * T) + 1), va[u + 4], vb[u + 4]);
+        }
+        wrote = true;
+    } else if (R0 == 4) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            ifft_bf4(va[u], va[u + 2], va[u + 4], va[u + 6]);
+            ifft_bf4(vb[u], vb[u + 2], vb[u + 4], vb[u + 6]);
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) put(ifft_row<PAD>(4 * (t + u * T) + r), va[u + 2 * r], vb[u + 2 * r]);
+        wrote = true;
+    }
+    if (wrote) {
+        __syncthreads();
+        const int rt = ifft_row<PAD>(t);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) get(ifft_row_at<PAD>(rt, t, q * T, T % (1 << PAD) == 0), va[q], vb[q]);
+    }
+#pragma unroll
+    for (int i = 0; i < N8; ++i) {
+        const int Ns = R0 << (3 * i);
+        const int k = t & (Ns - 1);
+        if (Ns > 1) {
+            const int step = L / (8 * Ns);
+            const float2 w1 = tw[k * step], w2 = tw[2 * k * step], w4 = tw[4 * k * step];
+            const float2 w3 = ACC ? tw[3 * k * step] : ifft_cmul(w1, w2);
+            const float2 w5 = ACC ? tw[5 * k * step] : ifft_cmul(w1, w4);
+            const float2 w6 = ACC ? tw[6 * k * step] : ifft_cmul(w2, w4);
+            const float2 w7 = ACC ? tw[7 * k * step] : ifft_cmul(w3, w4);
+            va[1] = ifft_cmul(va[1], w1); va[2] = ifft_cmul(va[2], w2); va[3] = ifft_cmul(va[3], w3);
+            va[4] = ifft_cmul(va[4], w4); va[5] = ifft_cmul(va[5], w5); va[6] = ifft_cmul(va[6], w6);
+            va[7] = ifft_cmul(va[7], w7);
+            vb[1] = ifft_cmul(vb[1], w1); vb[2] = ifft_cmul(vb[2], w2); vb[3] = ifft_cmul(vb[3], w3);
+            vb[4] = ifft_cmul(vb[4], w4); vb[5] = ifft_cmul(vb[5], w5); vb[6] = ifft_cmul(vb[6], w6);
+            vb[7] = ifft_cmul(vb[7], w7);
+        }
+        ifft_bf8(va);
+        ifft_bf8(vb);
+        const int j0 = (t - k) * 8 + k;
+        if (i == N8 - 1) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) emit(r, j0 + r * Ns, va[r], vb[r]);
+        } else {
+            if (wrote) __syncthreads();
+            {
+                const int rj = ifft_row<PAD>(j0);
+                const bool lin = Ns % (1 << PAD) == 0 || (Ns == 1 && PAD >= 3);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) put(ifft_row_at<PAD>(rj, j0, r * Ns, lin), va[r], vb[r]);
+            }
+            wrote = true;
+            __syncthreads();
+            {
+                const int rt = ifft_row<PAD>(t);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) get(ifft_row_at<PAD>(rt, t, q * T, T % (1 << PAD) == 0), va[q], vb[q]);
             }
         }
     }
@@ -238,7 +333,7 @@ __global__ void __launch_bounds__(256) k_ifft_tables(float2* tab, int lg1, int l
 #ifndef IFFT_MINB_B
 #define IFFT_MINB_B 2
 #endif
-template <int LG, int LGC>
+template <int LG, int LGC, bool ACC>
 __global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_A)
 k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict__ B, int lg2,
               const float2* __restrict__ tab)
@@ -290,18 +385,22 @@ k_ifft_pass_a(const float2* __restrict__ Y, long long ypitch, float2* __restrict
     }
     // e^{+2 pi i k2 n1 / M} for the outputs n1 = t + r L / 8 in turn: the first from the hi / lo tables, then
     // times colg[c] each
-    float2 pw = ifft_cmul(colt[c * W + (t >> 5)], colt[c * W + HI + (t & 31)]);
-    const float2 pg = colt[c * W + HI + 33];
     float2* bc = b + c0 + c;
-    ifft_core<LG, LGC, PAD>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
-        if (r > 0) pw = ifft_cmul(pw, pg);
+    // e^{+2 pi i k2 n1 / M} for the outputs n1 = t + r L / 8: a product of two table entries each (ACC), or the
+    // first one so and then times colg[c] each
+    const float2* ct = colt + c * W;
+    float2 pw = ifft_cmul(ct[t >> 5], ct[HI + (t & 31)]);
+    const float2 pg = ct[HI + 33];
+    ifft_core<LG, LGC, PAD, ACC>(v, s, tw, t, c, t, c, [&](int r, int n1, float2 val) {
+        if (ACC) pw = ifft_cmul(ct[n1 >> 5], ct[HI + (n1 & 31)]);
+        else if (r > 0) pw = ifft_cmul(pw, pg);
         bc[(long long)n1 << lg2] = ifft_cmul(val, pw);
     });
 }
 
 // Pass B.  grid = (M1 / C, rows), CTA = C rows n1 of B x L / 8 threads, L = M2 = 2^LG.
 // out: [rows][opitch] floats, the first nout of the 2 M samples.
-template <int LG, int LGC>
+template <int LG, int LGC, bool ACC>
 __global__ void __launch_bounds__(1 << (LG - 3 + LGC), (LG - 3 + LGC) >= 10 ? 1 : IFFT_MINB_B)
 k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long opitch, long long nout, int lg1,
               float mean, const float2* __restrict__ tab)
@@ -333,7 +432,7 @@ k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long o
     __syncthreads();
     // (rows of the caller's array may start on an odd float: then two 4-byte stores per point)
     const bool vec = (reinterpret_cast<uintptr_t>(o) & 7) == 0;
-    ifft_core<LG, LGC, PAD>(v, s, tw, t_in, c_in, t, c, [&](int, int n2, float2 val) {
+    ifft_core<LG, LGC, PAD, ACC>(v, s, tw, t_in, c_in, t, c, [&](int, int n2, float2 val) {
         const long long n = n1 + ((long long)n2 << lg1);                 // z[n] = (y[2n], y[2n+1])
         if (2 * n + 1 < nout) {
             if (vec) {
@@ -344,6 +443,58 @@ k_ifft_pass_b(const float2* __restrict__ B, float* __restrict__ out, long long o
             }
         } else if (2 * n < nout) {
             o[2 * n] = val.x + mean;
+        }
+    });
+}
+
+// Pass B with two transforms per thread: a CTA takes 8 rows n1 of B (threads: 4 row pairs x L / 8), so that
+// the stores are 64-byte runs (16 bytes per lane) and the loads 64-byte runs of each row.  Tile [rows][8]
+// float2, point i in row i + (i >> PAD), PAD = log2 of the first stage's radix: conflict-free for 16-byte
+// accesses (enumerated as for ifft_pad_a).
+__host__ __device__ constexpr int ifft_pad_b2(int lg) { return lg % 3 ? lg % 3 : 3; }
+constexpr size_t ifft_smem_b2(int lg)
+{
+    return ((size_t)((1 << lg) + ((1 << lg) >> ifft_pad_b2(lg))) * 8 + (size_t)(1 << lg)) * sizeof(float2);
+}
+
+template <int LG, bool ACC>
+__global__ void __launch_bounds__(1 << (LG - 1), LG >= 11 ? 1 : 2)
+k_ifft_pass_b2(const float2* __restrict__ B, float* __restrict__ out, long long opitch, long long nout, int lg1,
+               float mean, const float2* __restrict__ tab)
+{
+    constexpr int L = 1 << LG, T = L / 8, NT = T * 4, PAD = ifft_pad_b2(LG);
+    extern __shared__ __align__(16) float2 ifft_smem[];
+    float2* s = ifft_smem;                         // [L + (L >> PAD)][8]
+    float2* tw = s + (L + (L >> PAD)) * 8;         // [L]
+    const int c = threadIdx.x & 3, t = threadIdx.x >> 2;
+    const long long M = (long long)1 << (LG + lg1);
+    const long long n1 = (long long)blockIdx.x * 8 + 2 * c;
+    const float2* b0 = B + (long long)blockIdx.y * M + (n1 << LG);
+    float* o = out + (long long)blockIdx.y * opitch;
+    {
+        const float4* g = reinterpret_cast<const float4*>(tab + ((size_t)2 << lg1));
+        float4* d = reinterpret_cast<float4*>(tw);
+        for (int j = threadIdx.x; j < L / 2; j += NT) d[j] = __ldg(g + j);
+    }
+    float2 va[8], vb[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        va[q] = b0[t + q * T];
+        vb[q] = b0[L + t + q * T];
+    }
+    __syncthreads();
+    // z[n] = (y[2n], y[2n+1]); this thread's n and n + 1 are 16 contiguous bytes of the row
+    const bool vec = (reinterpret_cast<uintptr_t>(o) & 15) == 0;
+    ifft_core2<LG, 2, PAD, ACC>(va, vb, s, tw, t, c, [&](int, int n2, float2 a, float2 b) {
+        const long long n = n1 + ((long long)n2 << lg1);
+        float* p = o + 2 * n;
+        if (vec && 2 * n + 3 < nout) {
+            *reinterpret_cast<float4*>(p) = make_float4(a.x + mean, a.y + mean, b.x + mean, b.y + mean);
+        } else {
+            if (2 * n < nout) p[0] = a.x + mean;
+            if (2 * n + 1 < nout) p[1] = a.y + mean;
+            if (2 * n + 2 < nout) p[2] = b.x + mean;
+            if (2 * n + 3 < nout) p[3] = b.y + mean;
         }
     });
 }
@@ -372,36 +523,53 @@ inline int ifft_lgc(int lg)
     return lg <= 9 ? 3 : (lg == 10 && wide ? 3 : 2);
 }
 
-template <int LG, int LGC>
+template <int LG, int LGC, bool ACC>
 inline int ifft_launch_a(const float2* Y, long long ypitch, float2* B, int lg2, const float2* tab, int rows,
                          cudaStream_t s)
 {
     static bool attr = false;
     constexpr size_t bytes = ifft_smem_a(LG, LGC);
     if (!attr) {
-        if (cudaFuncSetAttribute(k_ifft_pass_a<LG, LGC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
+        if (cudaFuncSetAttribute(k_ifft_pass_a<LG, LGC, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
             cudaSuccess)
             return -3;
         attr = true;
     }
-    k_ifft_pass_a<LG, LGC><<<dim3((unsigned)((1 << lg2) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
+    k_ifft_pass_a<LG, LGC, ACC><<<dim3((unsigned)((1 << lg2) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
         Y, ypitch, B, lg2, tab);
     return 0;
 }
 
-template <int LG, int LGC>
+template <int LG, int LGC, bool ACC>
 inline int ifft_launch_b(const float2* B, float* out, long long opitch, long long nout, int lg1, float mean,
                          const float2* tab, int rows, cudaStream_t s)
 {
     static bool attr = false;
     constexpr size_t bytes = ifft_smem_b(LG, LGC);
     if (!attr) {
-        if (cudaFuncSetAttribute(k_ifft_pass_b<LG, LGC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
+        if (cudaFuncSetAttribute(k_ifft_pass_b<LG, LGC, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
             cudaSuccess)
             return -3;
         attr = true;
     }
-    k_ifft_pass_b<LG, LGC><<<dim3((unsigned)((1 << lg1) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
+    k_ifft_pass_b<LG, LGC, ACC><<<dim3((unsigned)((1 << lg1) >> LGC), (unsigned)rows), 1 << (LG - 3 + LGC), bytes, s>>>(
+        B, out, opitch, nout, lg1, mean, tab);
+    return 0;
+}
+
+template <int LG, bool ACC>
+inline int ifft_launch_b2(const float2* B, float* out, long long opitch, long long nout, int lg1, float mean,
+                          const float2* tab, int rows, cudaStream_t s)
+{
+    static bool attr = false;
+    constexpr size_t bytes = ifft_smem_b2(LG);
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_ifft_pass_b2<LG, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) !=
+            cudaSuccess)
+            return -3;
+        attr = true;
+    }
+    k_ifft_pass_b2<LG, ACC><<<dim3((unsigned)((1 << lg1) >> 3), (unsigned)rows), 1 << (LG - 1), bytes, s>>>(
         B, out, opitch, nout, lg1, mean, tab);
     return 0;
 }
@@ -434,29 +602,44 @@ inline int ifft_make_tables(long long nfft_out, float2* tab, cudaStream_t s)
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
 }
 
-// rows of Y -> rows of out, in launches of `batch` rows through the intermediate `ring` ([batch][M] float2)
-inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
-                       long long nfft_out, float mean, float2* ring, const float2* tab, int batch, cudaStream_t s)
+template <bool ACC>
+inline int ifft_launch_acc(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
+                           int lg1, int lg2, float mean, float2* ring, const float2* tab, int batch, cudaStream_t s)
 {
-    int M1, M2;
-    if (!ifft_split(nfft_out, &M1, &M2)) return -5;
-    const long long M = (long long)M1 * M2;
-    int lg1 = 0, lg2 = 0;
-    while ((1 << lg1) < M1) ++lg1;
-    while ((1 << lg2) < M2) ++lg2;
     const int lgc1 = ifft_lgc(lg1), lgc2 = ifft_lgc(lg2);
-    (void)M;
     for (int r0 = 0; r0 < rows; r0 += batch) {
         const int n = rows - r0 < batch ? rows - r0 : batch;
         float2* b = ring;
         int rc = 0;
-        FDD_IFFT_DISPATCH(lg1, lgc1, (rc = ifft_launch_a<LG_, LGC_>(Y + (long long)r0 * ypitch, ypitch, b, lg2, tab, n, s)));
+        FDD_IFFT_DISPATCH(lg1, lgc1,
+                          (rc = ifft_launch_a<LG_, LGC_, ACC>(Y + (long long)r0 * ypitch, ypitch, b, lg2, tab, n, s)));
         if (rc != 0) return rc;
-        FDD_IFFT_DISPATCH(lg2, lgc2, (rc = ifft_launch_b<LG_, LGC_>(b, out + (long long)r0 * opitch, opitch, nout,
-                                                                     lg1, mean, tab, n, s)));
+        // pass B with two transforms per thread for 2048-point transforms (the paper's 2^23-point series:
+        // a5 55.1 ms against 57.8 at 1024 trial DMs; at 1024 points it has fewer instructions and wavefronts
+        // but too few warps to hide the exchanges: 19.2 against 18.8 ms, so those keep one per thread)
+        float* o = out + (long long)r0 * opitch;
+        if (lg2 == 11) rc = ifft_launch_b2<11, ACC>(b, o, opitch, nout, lg1, mean, tab, n, s);
+        else
+            FDD_IFFT_DISPATCH(lg2, lgc2,
+                              (rc = ifft_launch_b<LG_, LGC_, ACC>(b, o, opitch, nout, lg1, mean, tab, n, s)));
         if (rc != 0) return rc;
     }
     return cudaGetLastError() == cudaSuccess ? 0 : -3;
+}
+
+// rows of Y -> rows of out, in launches of `batch` rows through the intermediate `ring` ([batch][M] float2);
+// accurate: the form with every twiddle from a table (zero-padded series, see ifft_core)
+inline int ifft_launch(const float2* Y, long long ypitch, int rows, float* out, long long opitch, long long nout,
+                       long long nfft_out, float mean, float2* ring, const float2* tab, int batch, bool accurate,
+                       cudaStream_t s)
+{
+    int M1, M2;
+    if (!ifft_split(nfft_out, &M1, &M2)) return -5;
+    int lg1 = 0, lg2 = 0;
+    while ((1 << lg1) < M1) ++lg1;
+    while ((1 << lg2) < M2) ++lg2;
+    return accurate ? ifft_launch_acc<true>(Y, ypitch, rows, out, opitch, nout, lg1, lg2, mean, ring, tab, batch, s)
+                    : ifft_launch_acc<false>(Y, ypitch, rows, out, opitch, nout, lg1, lg2, mean, ring, tab, batch, s);
 }
 
 }  // namespace fdd
