@@ -819,6 +819,11 @@ def test_inverse_transform_choices(F, oracle_c, nchans, nsamps, ndm, step, kerne
             if which != F.FDD_INVERSE_AUTO:
                 # (every length here is one the hand-written inverse takes)
                 assert plan.get_inverse() == which
+            else:
+                # AUTO: cuFFT's half-length C2C behind SYMMETRIC2's fused pre-twiddle (not for zero-padded
+                # series, whose a4 writes plain sums), the hand-written inverse behind every other kernel
+                fused = plan.get_info()[5] == F.FDD_KERNEL_SYMMETRIC2 and nsamps & (nsamps - 1) == 0
+                assert plan.get_inverse() == (F.FDD_INVERSE_CUFFT if fused else F.FDD_INVERSE_TWO_PASS)
             worst = parity.assert_rows(got, ref, "time", f"inverse {which}/{kernel}/{nchans}x{nsamps}")
             print("inverse", which, kernel, nchans, nsamps, worst)
         with pytest.raises(F.FddError):
