@@ -9,6 +9,7 @@ import pytest
 
 import parity
 import synth
+from oracle import fdd_oracle as O
 
 pytestmark = pytest.mark.gpu
 
@@ -52,7 +53,7 @@ def _static_path(F, plan, x_dev, pitch, dc_add, delays, poison=False):
     return o[..., 0] + 1j * o[..., 1]
 
 
-def test_static_scratch_entry_point_matches_the_plan_path_on_calls_in_a_row(F):
+def test_static_scratch_entry_point_matches_the_plan_path_on_calls_in_a_row(F, oracle_c):
     # A: 40 trial DMs (5 DM tiles), 4097 bins (a ragged tail of the 128-bin CTAs); B: fewer, other delays,
     # 13 trial DMs (a ragged DM tile) - the static table still holds A's entries when B runs
     wa = synth.small_workload(4100, 64, 8192, 40, dm_step=1.5)
@@ -64,6 +65,13 @@ def test_static_scratch_entry_point_matches_the_plan_path_on_calls_in_a_row(F):
             got = _static_path(F, plan, x_dev, pitch, dc_add, delays, poison=True)
             assert np.isfinite(got.view(np.float64)).all(), f"call {rnd}: output rows not written"
             worst = parity.assert_rows(got, ref, "fourier", f"static scratch, call {rnd}")
+            if rnd < 2:
+                # ... and against the oracle itself (Eq. 4 + 7), the bar of every parity test
+                w = (wa, wb)[rnd]
+                rows = list(range(plan.ndm))
+                exact = O.fdd_rows(synth.make_filterbank(w), O.delay_table(w.nchans, w.f_lo, w.f_hi, w.tsamp,
+                                                                         w.dm_list), rows, mode="fourier")
+                parity.assert_rows(got, exact, "fourier", f"static scratch against the oracle, call {rnd}")
             # the same 64-bit phase table on both sides (the plan's kernel walks the bins by a recurrence,
             # this one makes a fresh phasor per element): measured 3e-7, far inside the bar
             assert worst["rel_l2"] <= 1e-5, (rnd, worst)
