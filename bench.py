@@ -535,7 +535,10 @@ def run_b200(args, rank: int, local_rank: int, world: int):
             nlaunch = -(-w.ndm // 4096)
         kpad = -(-w.nchans // 64) * 64
         bpad = -(-nbins // 4) * 4
-        mma_flop = nlaunch * 3.0 * 2.0 * 128 * 64 * kpad * bpad
+        # a one-beam launch of <= 2048 trial DMs takes 64 operand rows (UMMA M = 64: half the flop of the
+        # 128-row form in the same tensor-pipe time - the pipe's peak is then out of reach by design)
+        mrows = 64 if (nbeams == 1 and w.ndm <= 2048 and os.environ.get("FDD_TC_FEW") != "0") else 128
+        mma_flop = nlaunch * 3.0 * 2.0 * mrows * 64 * kpad * bpad
         roofline.update({
             "bound": "tensor", "achieved": mma_flop / (sum_ms * 1e-3) * 1e-12, "peak": tpeak,
             "frac": mma_flop / (sum_ms * 1e-3) * 1e-12 / tpeak,
@@ -543,7 +546,7 @@ def run_b200(args, rank: int, local_rank: int, world: int):
                             "loop; fp16 and bf16 share the kind::f16 rate); burst figure "
                             f"{pk.get('bf16_tflops')}") if pk else
                            "fallback 1.4 PFLOP/s sustained (B200_PROFILING.md): MEASURED_PEAKS.json absent",
-            "achieved_is": "executed tcgen05.mma flop (3 fp16 products of 128 x 64 x N_nu per bin and "
+            "achieved_is": f"executed tcgen05.mma flop (3 fp16 products of {mrows} x 64 x N_nu per bin and "
                            "launch) / mean launch duration (CUDA events around the stage)",
             "fp32_peak_tflops_measured": peak_tf,
             "algorithmic_equiv_over_fp32_peak": FLOP_PER_ELEMENT * elements / (sum_ms * 1e-3) * 1e-12 / peak_tf,

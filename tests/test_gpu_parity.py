@@ -716,12 +716,19 @@ def test_tensor_core_conventions_selftest(F):
     (100, 4096, 200, 0.3),           # ragged channels (two 64-channel stages, 28 padded), 3 tiles + 8 rows
     (256, 1000, 4096, 0.02),         # all 64 tiles, padded series (1000 -> 1024), last item 1 live bin
     (1024, 2048, 300, 0.05),         # the most channels the kernel stages
+    # launches of <= 32 tiles take 64 operand rows (UMMA M = 64) and share the generator warps differently
+    (64, 2048, 1000, 0.05),          # 16 tiles: both 8-tile halves of the one Z warp live
+    (128, 1024, 1500, 0.03),         # 24 tiles: 16-tile halves, the second one half live
+    (64, 1024, 2048, 0.02),          # 32 tiles, the most of that form
+    (64, 1024, 2100, 0.02),          # 33 tiles: the 128-row form again
 ])
 def test_tensor_core_kernel_against_the_oracle(F, oracle_c, nchans, nsamps, ndm, step, mode):
     w = synth.small_workload(600 + nchans, nchans, nsamps, ndm, dm_step=step, mode=mode)
     u8 = synth.make_filterbank(w)
     d = _delays_for(w)
-    rows = list(range(ndm)) if ndm <= 300 else sorted(set(range(0, ndm, 61)) | {31, 32, 63, 64, ndm - 1})
+    rows = list(range(ndm)) if ndm <= 300 else sorted(
+        set(range(0, ndm, 61)) | {31, 32, 63, 64, ndm - 1} |
+        {j for j in (511, 512, 543, 1023, 1024, 1055, 1535, 1536, 2047, 2048, 2079) if j < ndm})
     ref = O.fdd_rows(u8, d, rows, mode=mode)
     with _plan_for(F, w) as plan:
         plan.set_kernel(F.FDD_KERNEL_TENSOR)
