@@ -69,6 +69,8 @@ def parse_args():
                          "input, the others seeded noise made on the device); the rate counts all beams")
     ap.add_argument("--inverse", default="auto", choices=["auto", "cufft", "two_pass"],
                     help="step a5: the plan's choice (default), cuFFT, or the hand-written two-pass inverse")
+    ap.add_argument("--y-budget-gib", type=float, default=0.0, metavar="G",
+                    help="fdd_plan_set_y_budget: TIME-mode Y scratch per DM chunk (0 = the library's default)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -319,6 +321,8 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     nfft, nbins, valid, maxd, scratch, kernel = plan.get_info()
     if args.decimate:
         plan.set_decimation(args.decimate)
+    if args.y_budget_gib > 0:
+        plan.set_y_budget(int(args.y_budget_gib * (1 << 30)))
     if args.inverse != "auto":
         plan.set_inverse(F.FDD_INVERSE_TWO_PASS if args.inverse == "two_pass" else F.FDD_INVERSE_CUFFT)
     ns_out, nbins = plan.output_shape()                   # = (nsamps, nbins) at full rate
@@ -370,6 +374,9 @@ def run_b200(args, rank: int, local_rank: int, world: int):
     sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
     stage_ms, launches = plan.get_stage_ms()
+    # (a TIME-mode plan whose Y chunks are short falls back to the FP32 kernel at its first execute:
+    #  report the kernel that ran, and the scratch it holds now)
+    scratch, kernel = plan.get_info()[4:6]
     own_inverse = mode == F.FDD_MODE_TIME and plan.get_inverse() == F.FDD_INVERSE_TWO_PASS
     plan.set_profiling(False)
     if flush is not None:                                  # the flush is not part of the path
@@ -570,7 +577,9 @@ def run_b200(args, rank: int, local_rank: int, world: int):
                               if not k.startswith("tdd_")},
         "roofline": roofline,
         "plan": {"nfft": nfft, "nbins": nbins, "valid_len": valid, "max_delay_samples": maxd,
-                 "scratch_bytes": scratch, "kernel": kernel},
+                 "scratch_bytes": scratch, "kernel": kernel,
+                 "rotate_sum_chunks_per_step": launches["rotate_sum"] / args.steps,
+                 "device_free_bytes": torch.cuda.mem_get_info()[0]},
     }
     # HBM-bound stages: achieved GB/s against the measured copy bandwidth
     peaks = {}

@@ -148,9 +148,10 @@ int fdd_plan_get_output_shape(const fdd_plan *plan, long long *nsamps_out, long 
  * or FDD_KERNEL_SYMMETRIC2 for a delay table that is not in arithmetic progression within every
  * 32-DM tile (tiles count from the first trial DM), or if FDD_KERNEL_TENSOR is asked for a table that
  * is not ONE progression over all trial DMs (or has more than 1024 channels, or nfft > 2^23).  AUTO
- * takes the fastest kernel the table allows: TENSOR (uniform DM grids with at least 1024 trial DMs -
- * its cost does not depend on the number of trial DMs of a launch, up to 4096; a TIME-mode plan whose
- * sums must be processed in chunks of fewer than 1024 rows stays on SYMMETRIC2), else
+ * takes the fastest kernel the table allows: TENSOR (uniform DM grids with at least 640 trial DMs -
+ * its cost is the same for any number of trial DMs of a launch up to 1024, up to 2048 and up to 4096
+ * (64 or 128 operand rows); a TIME-mode plan whose sums must be processed in chunks of fewer than
+ * 640 rows stays on SYMMETRIC2), else
  * SYMMETRIC2 (uniform DM grids, and piecewise-uniform DM plans whose segments are multiples
  * of 32 trial DMs), MIXED (piecewise-uniform plans with any segment lengths: only the tiles that
  * contain a step change run on the about 3.5 times slower generic kernel; at least half of the
@@ -161,7 +162,7 @@ int fdd_plan_set_kernel(fdd_plan *plan, int kernel);
 /* Make everything an fdd_execute / fdd_rotate_sum_only in `mode` (enum fdd_mode) needs that the plan
  * creates lazily, so that the execute itself allocates nothing, uploads nothing and never
  * synchronises (it can then be captured in a CUDA graph):
- *   TIME     the Y scratch (up to 24 GiB, see fdd_plan_set_y_budget), the inverse cuFFT plans and
+ *   TIME     the Y scratch (up to 24 GiB, 64 GiB on FDD_KERNEL_TENSOR; see fdd_plan_set_y_budget), the inverse cuFFT plans and
  *            the shared cuFFT workspace
  *   both     the bin-recurrence tables if any trial DM runs on FDD_KERNEL_GENERIC, the launch
  *            shapes (DM-tile groups) of the shared-recurrence kernel, and the fp64 table of a
@@ -181,8 +182,8 @@ int fdd_plan_set_inverse(fdd_plan *plan, int which);
 int fdd_plan_get_inverse(const fdd_plan *plan, int *which);
 
 /* TIME mode keeps the sums Y of a chunk of trial DMs in plan-owned scratch between a4 and a5.  The
- * chunk is as many rows as fit `bytes` (default 24 GiB, and never more than half of the free
- * device memory), rounded down to whole inverse-FFT batches (384 rows), 96-DM groups, 32-DM tiles
+ * chunk is as many rows as fit `bytes` (default 24 GiB - 64 GiB for a plan on FDD_KERNEL_TENSOR, whose
+ * cost is per launch, not per row - and never more than half of the free device memory), rounded down to whole inverse-FFT batches (384 rows), 96-DM groups, 32-DM tiles
  * or multiples of 8 rows; plans with more trial DMs run a4 + a5 chunk after chunk (the paper's
  * DM_outer batches, without re-doing a2 + a3).  bytes = 0 restores the default.
  * FDD_ERR_ALLOC from the next TIME execute / prepare if not even 8 rows fit.  Synchronises the

@@ -30,6 +30,10 @@ namespace {
 constexpr double kDefaultKdm = 4.148808e3;            // MHz^2 pc^-1 cm^3 s (reading S5)
 constexpr long long kPitchAlign = 16;                 // float2 elements (128 B)
 constexpr size_t kYBudgetBytes = (size_t)24 << 30;    // TIME-mode Y scratch per DM chunk
+// ... of a plan on the tensor-core kernel, whose cost is per launch, not per row (measured at the
+// paper's shape, 1024 channels x 2^23 points x 1024 trial DMs: one launch 219 ms, three 384-row chunks
+// 660 ms, the FP32 kernel 377 ms): room for 2048 rows of 2^23 points
+constexpr size_t kYBudgetTensorBytes = ((size_t)64 << 30) + ((size_t)1 << 27);
 constexpr int kC2RBatch = 384;                        // rows per cuFFT inverse call (4 x 96-DM groups)
 constexpr int kHostChunkRows = kC2RBatch;             // fdd_execute_host: DM rows per pipelined chunk
 constexpr int kHostRingChunks = 3;                    // fdd_execute_host: output chunks resident on the device
@@ -47,7 +51,10 @@ int ifft_batch(long long nfft_out)
     const long long rows = (1LL << 26) / (nfft_out / 2 > 0 ? nfft_out / 2 : 1);
     return rows < 8 ? 8 : (rows > 512 ? 512 : (int)rows);
 }
-constexpr int kTensorMinRows = 1024;                  // launches with fewer trial DMs take the FP32 kernels
+// AUTO: launches with fewer trial DMs take the FP32 kernels.  Measured on B200 (1024 channels x 2^20
+// samples): the tensor-core kernel's 64-row form costs 27.4 ms for any number of trial DMs up to 1024,
+// the shared-recurrence kernel 25.9 ms at 512 and 47 ms at 1024 (proportional to the rows).
+constexpr int kTensorMinRows = 640;
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
@@ -226,9 +233,9 @@ int resolve_kernel(const fdd_plan* p, int request)
         case FDD_KERNEL_MIXED: return sym2_ok ? FDD_KERNEL_SYMMETRIC2
                                               : (any_ap ? FDD_KERNEL_MIXED : FDD_KERNEL_GENERIC);
         default:
-            // measured on B200 (1024 channels x 2^20 samples): the tensor-core kernel costs the same
-            // for any number of trial DMs up to 4096 per launch (43 ms), the shared-recurrence kernel
-            // 46 ms per 1024 trial DMs
+            // measured on B200 (1024 channels x 2^20 samples): the tensor-core kernel costs 27 ms up to
+            // 1024 trial DMs per launch, 36 ms up to 2048 and 46 ms up to 4096, the shared-recurrence
+            // kernel 46 ms per 1024 trial DMs
             if (tensor_ok(p) && p->ndm >= kTensorMinRows) return FDD_KERNEL_TENSOR;
             if (sym2_ok) return FDD_KERNEL_SYMMETRIC2;
             // a few tiles hold a change of DM step: those rows alone take the generic kernel
@@ -376,7 +383,9 @@ int ensure_time_resources(fdd_plan* p, int family)
     if (!p->Y) {
         p->ypitch = round_up(p->nbins_out, kPitchAlign);
         const size_t row_bytes = (size_t)p->ypitch * sizeof(float2);
-        long long rows = (long long)((p->y_budget ? p->y_budget : kYBudgetBytes) / row_bytes);
+        const size_t budget = p->y_budget ? p->y_budget
+                                          : (p->kernel == FDD_KERNEL_TENSOR ? kYBudgetTensorBytes : kYBudgetBytes);
+        long long rows = (long long)(budget / row_bytes);
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
             long long fit = (long long)(free_b / 2 / row_bytes);
