@@ -52,7 +52,7 @@ int ifft_batch(long long nfft_out)
     return rows < 8 ? 8 : (rows > 512 ? 512 : (int)rows);
 }
 // AUTO: launches with fewer trial DMs take the FP32 kernels.  Measured on B200 (1024 channels x 2^20
-// samples): the tensor-core kernel's 64-row form costs 27.4 ms for any number of trial DMs up to 1024,
+// samples): the tensor-core kernel's 64-row form costs 26.9 ms for any number of trial DMs up to 1024,
 // the shared-recurrence kernel 25.9 ms at 512 and 47 ms at 1024 (proportional to the rows).
 constexpr int kTensorMinRows = 640;
 
