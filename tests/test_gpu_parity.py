@@ -52,7 +52,7 @@ KERNELS = ["generic", "symmetric", "auto"]
 
 
 def _set_kernel(F, plan, which):
-    """auto = the fastest kernel the delay table allows (on uniform DM grids SYMMETRIC2 below 1024
+    """auto = the fastest kernel the delay table allows (on uniform DM grids SYMMETRIC2 below 640
     trial DMs, TENSOR from there).  Returns the kernel the plan resolved to (enum fdd_kernel)."""
     plan.set_kernel({"generic": F.FDD_KERNEL_GENERIC, "symmetric": F.FDD_KERNEL_SYMMETRIC,
                      "symmetric2": F.FDD_KERNEL_SYMMETRIC2, "tensor": F.FDD_KERNEL_TENSOR,
@@ -736,6 +736,23 @@ def test_tensor_core_kernel_against_the_oracle(F, oracle_c, nchans, nsamps, ndm,
         got = _run(F, plan, u8, mode)[rows]
     worst = parity.assert_rows(got, ref, mode, f"tensor {nchans}x{nsamps}x{ndm}/{mode}")
     print("tensor", nchans, nsamps, ndm, mode, worst)
+
+
+@pytest.mark.parametrize("ndm,want", [(608, "symmetric2"), (640, "tensor")])
+def test_auto_takes_the_tensor_kernel_from_640_trial_dms(F, oracle_c, ndm, want):
+    """AUTO on a uniform DM grid: the FP32 shared-recurrence kernel below 640 trial DMs, the
+    tensor-core kernel (its 64-row form) from there - each against the oracle, TIME mode, so that the
+    a5 behind either kernel is part of the check."""
+    w = synth.small_workload(640 + ndm, 48, 2048, ndm, dm_step=0.04, mode="time")
+    u8 = synth.make_filterbank(w)
+    d = _delays_for(w)
+    rows = sorted(set(range(0, ndm, 53)) | {31, 32, 511, 512, ndm - 1})
+    ref = O.fdd_rows(u8, d, rows, mode="time")
+    with _plan_for(F, w) as plan:
+        assert plan.get_info()[5] == {"symmetric2": F.FDD_KERNEL_SYMMETRIC2, "tensor": F.FDD_KERNEL_TENSOR}[want]
+        got = _run(F, plan, u8, "time")[rows]
+        assert plan.get_info()[5] == {"symmetric2": F.FDD_KERNEL_SYMMETRIC2, "tensor": F.FDD_KERNEL_TENSOR}[want]
+    parity.assert_rows(got, ref, "time", f"auto at {ndm} trial DMs")
 
 
 # ------------------------------------------------------------------ row f1: several beams, one plan
